@@ -1,0 +1,137 @@
+/* gst.h -- C ABI of the B200-native spin-orbit tracker (after arXiv:1501.03450, GPUSPINTRACK).
+ *
+ * The library tracks a bunch of spin-1/2 particles, one CUDA thread per particle, through
+ * a ring lattice for many turns: symplectic orbital integration through every element
+ * (section 3) followed by Thomas-BMT spin integration with quaternions and Romberg
+ * extrapolation (section 4).  "P:nnn" cites /root/reference/PAPER.md line nnn; "(n)" an equation.
+ *
+ * Conventions
+ *   - Phase space is MAD's canonical set (1) P:55: X, Px, Y, Py, T = -c dt, Pt = (E-E0)/(p0 c);
+ *     momenta in units of the reference momentum p0.  Spin is a unit 3-vector with
+ *     components along the local (x, y, s) axes: x radial-outward, y up, s along the beam.
+ *   - All particle data are fp64, structure-of-arrays, in DEVICE memory owned by the caller
+ *     (e.g. torch tensors); the library borrows the nine pointers and updates them in place.
+ *   - Opaque handles; every call returns a gst_status; no exceptions or aborts cross the ABI.
+ *     gst_last_error() gives a thread-local message for the last non-OK status.
+ *   - Nothing here falls back to the CPU: without a CUDA device every compute call returns
+ *     GST_ECUDA.
+ */
+#ifndef GST_H_
+#define GST_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum { GST_OK = 0, GST_EINVAL = 1, GST_ENOMEM = 2, GST_ECUDA = 3, GST_ESTATE = 4 } gst_status;
+
+/* element types: P:114-464 (orbit), P:585 (snake); RFCAV is DESIGN.md reading A12/A13 */
+typedef enum {
+  GST_DRIFT = 0,     /* exact drift, flow of H_drift (29b) P:371                                   */
+  GST_SBEND = 1,     /* sector bend: exact flow (10) P:137, or TEAPOT drift-kick (30)(31) P:381     */
+  GST_QUAD = 2,      /* quadrupole: matrix-kick (24)(25)(27) P:298-353, or drift-kick (29)          */
+  GST_MULTIPOLE = 3, /* thick straight multipole, always drift-kick (28)(29) P:359-374              */
+  GST_THINMULT = 4,  /* thin lens, "drift-kick without the drift" P:378                             */
+  GST_RFCAV = 5,     /* thin RF cavity with optional reference-energy ramp                          */
+  GST_SNAKE = 6,     /* Siberian snake: orbit-transparent thin spin rotation P:585                  */
+  GST_MARKER = 7
+} gst_elem_type;
+
+/* which integrator each thick magnet uses (".apdf"; reading A16) */
+typedef enum {
+  GST_SPLIT_DRIFT_KICK = 0,  /* bends (30)(31), quads and multipoles (29)           */
+  GST_SPLIT_BEND_KICK = 1,   /* bends exact (10), quads and multipoles (29)         */
+  GST_SPLIT_MATRIX_KICK = 2  /* bends exact (10), quads (24)(25)(27): paper's BK/MK */
+} gst_split;
+
+/* One lattice element.  Plain data, 144 bytes, HOST memory, copied by gst_lattice_create.
+ * Strengths are normalised by the reference rigidity (B rho)_o = p0/q, so no rigidity is needed. */
+typedef struct {
+  int32_t type;       /* gst_elem_type                                                            */
+  int32_t slice_mult; /* thick magnets: slices = n_slices * slice_mult ("4 n_b"); >= 1      */
+  double L;           /* length [m]; > 0 for DRIFT/SBEND/QUAD/MULTIPOLE, ignored otherwise        */
+  double h;           /* SBEND: curvature of the local frame 1/rho_c = angle/L [1/m]; != 0 */
+  double k0;          /* SBEND: b1/(B rho)_o = eta*h [1/m] (9); eta != 1 is a mis-powered magnet  */
+  double kn[4];       /* normal  b_m/(B rho)_o, m = 2..5 -> kn[m-2], convention of (28): no 1/(m-1)!;
+                         QUAD uses kn[0] only (!= 0); THINMULT: integrated (times L)             */
+  double ks[4];       /* skew    a_m/(B rho)_o, same layout; must be 0 for QUAD                   */
+  double volt_eV;     /* RFCAV: q*V peak energy gain [eV]                                         */
+  double harmonic;    /* RFCAV: harmonic number; k_rf = 2 pi harmonic beta_o / C, C = sum of L    */
+  double phi_s;       /* RFCAV: synchronous phase [rad]; reference energy += volt_eV*sin(phi_s)   */
+  double sign;        /* RFCAV: +1/-1, dE = volt_eV*sin(phi_s + sign*k_rf*T)  (+1 above transition) */
+  double snake_mu;    /* SNAKE: rotation angle [rad]                                              */
+  double snake_phi;   /* SNAKE: axis (sin phi, 0, cos phi) in (x,y,s): angle from s-hat in the x-s plane */
+} gst_element;
+
+typedef struct {
+  double G;       /* gyromagnetic anomaly (g-2)/2 (4) P:87 */
+  double mass_eV; /* rest energy [eV]                       */
+  double gamma0;  /* reference Lorentz factor at turn 0     */
+} gst_beam; /* charge +1 */
+
+typedef struct gst_lattice gst_lattice;
+typedef struct gst_bunch gst_bunch;
+
+/* Stage an element table (a0).  `elems` and `beam` are HOST pointers, copied.  The table is
+ * de-duplicated to unique elements + a uint16 sequence and uploaded to the current CUDA device.
+ * GST_EINVAL: n == 0, unknown type, L <= 0 for a thick element, SBEND with h == 0 or k0 == 0, QUAD
+ * with kn[0] == 0 or any skew/higher term, slice_mult < 1, more than 65535 unique elements.      */
+gst_status gst_lattice_create(const gst_element* elems, size_t n, const gst_beam* beam, gst_lattice** out);
+void gst_lattice_destroy(gst_lattice* lat);
+
+/* particle-element-steps one particle makes per turn at `n_slices` (thick: n_slices*slice_mult,
+ * everything else 1): the unit of BASELINE.json's metric.                                          */
+int64_t gst_lattice_steps_per_turn(const gst_lattice* lat, int n_slices);
+
+/* Bind nine DEVICE arrays of n doubles each (SoA; D1, D2 of DESIGN.md).  Borrowed, not copied: the
+ * caller keeps them alive until gst_bunch_destroy.  Allocates the per-particle lost flags (A15).  */
+gst_status gst_bunch_init(double* x, double* px, double* y, double* py, double* t, double* pt, double* sx, double* sy,
+                          double* ss, size_t n, gst_bunch** out);
+void gst_bunch_destroy(gst_bunch* b);
+
+/* Track the bunch for n_turns turns of `lat` in place (a1-a12, a14).  ASYNCHRONOUS on
+ * `cuda_stream` (a cudaStream_t, NULL = default stream); never synchronises.  One launch of the
+ * persistent turn-loop kernel.  The bunch carries the turn counter and the reference energy across
+ * calls (first call takes gamma0 from the lattice's beam).
+ *   n_slices      base number of orbital slices per thick magnet (n_b of P:585), >= 1
+ *   romberg_depth number d of step-size levels in the Romberg table (39): 1 = trapezoid edge
+ *                 product only; d = k+1 for the paper's "k Romberg iterations"; 1..6
+ * GST_EINVAL if 2^(d-1) does not divide n_slices*slice_mult of some thick magnet (reading A4).   */
+gst_status gst_track(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, gst_split split, int n_slices,
+                     int romberg_depth, void* cuda_stream);
+
+/* Bunch polarization (a13; reading A18): out = {Px, Py, Ps, |P|} over particles not lost;
+ * out_lost (may be NULL) = number lost.  Enqueues the reduction on the stream and SYNCHRONISES it.
+ * `out` and `out_lost` are HOST pointers.                                                           */
+gst_status gst_polarization(gst_bunch* b, void* cuda_stream, double out[4], int64_t* out_lost);
+
+/* Geometric rms emittances (a13; reading A19), HOST out = {eps_x, eps_y}; synchronises the stream. */
+gst_status gst_emittance(gst_bunch* b, void* cuda_stream, double out_exy[2]);
+
+/* Copy the lost flags (1 = lost) to HOST memory, n bytes; synchronises the stream.                */
+gst_status gst_bunch_lost(gst_bunch* b, void* cuda_stream, uint8_t* host_out);
+
+/* Reference Lorentz factor and turn counter the bunch carries (host-side bookkeeping of A13).    */
+gst_status gst_bunch_reference(const gst_bunch* b, double* gamma0, int64_t* turn);
+gst_status gst_bunch_set_reference(gst_bunch* b, const gst_beam* beam, int64_t turn);
+
+/* End-to-end convenience with HOST buffers: allocates device arrays, copies the nine host arrays
+ * (n doubles each, pinned or pageable) to the device, tracks, reduces, copies the state back into
+ * the same host arrays and frees.  out_pol = {Px,Py,Ps,|P|}, out_lost may be NULL.  Synchronous.  */
+gst_status gst_track_host(const gst_lattice* lat, double* const host_state[9], size_t n, int64_t n_turns,
+                          gst_split split, int n_slices, int romberg_depth, double out_pol[4], int64_t* out_lost);
+
+/* Register-resident DFMA-chain microbenchmark on every SM of the current device: the measured
+ * FP64 (CUDA-core) peak the roofline is reported against.  HOST out: TFLOP/s (2 flop per DFMA).   */
+gst_status gst_fp64_peak(double* out_tflops, double* out_ms);
+
+/* Thread-local message for the last error on this thread; never NULL. */
+const char* gst_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GST_H_ */

@@ -1,0 +1,289 @@
+"""GPU parity: the CUDA path, called through the C ABI (ctypes binding), against the CPU oracle on the
+same seeded inputs, element by element.
+
+Metric: for an orbit coordinate c, max_j |gpu - oracle| / max_j |oracle_c|
+(bunch-scale relative; T is ~0 at turn 0 so per-value relative error is meaningless); for spin
+components, absolute.  Tolerances from BASELINE.json north_star: 1e-12 after one turn, 1e-9 after
+100 turns; bunch polarization within 1e-6 for the near-resonance and ramp configs.
+The oracle runs its literal formulas in long double (see gst_oracle.hpp header).
+"""
+import math
+
+import numpy as np
+import pytest
+
+from paper_1501_03450_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def gst():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1501_03450_b200 import gst as g
+    g.lib()
+    return g
+
+
+@pytest.fixture(scope="module")
+def O():
+    from oracle import oracle
+    oracle.lib()
+    return oracle
+
+
+def gpu_track(gst, lat, beam, state, n_turns, split, n_slices, depth, chunks=None):
+    L = gst.Lattice(lat, beam)
+    d = torch.tensor(state, dtype=torch.float64, device="cuda").contiguous()
+    b = gst.Bunch(d)
+    for nt in (chunks or [n_turns]):
+        b.track(L, nt, split, n_slices, depth)
+    pol, nlost = b.polarization()
+    emit = b.emittance()
+    lost = b.lost()
+    g1, turn = b.reference()
+    assert turn == n_turns
+    out = d.cpu().numpy()
+    b.close()
+    L.close()
+    return out, lost, pol, emit, g1
+
+
+def orbit_err(got, ref):
+    return max(np.max(np.abs(got[c] - ref[c])) / max(np.max(np.abs(ref[c])), 1e-300) for c in range(6))
+
+
+def spin_err(got, ref):
+    return float(np.max(np.abs(got[6:9] - ref[6:9])))
+
+
+def mixed_lattice(ramp=True):
+    """Every element type, both quad signs, a mis-powered bend, skew terms, slice multipliers."""
+    ang = 2 * math.pi / 24
+    els = [W.drift(0.7), W.quad(0.6, +0.35), W.thin_sextupole(0.4), W.drift(0.4),
+           W.sbend(1.8, ang, eta=1.0), W.snake(math.pi, math.radians(45)),
+           W.multipole(0.3, kn=(0.02, 0.9, -4.0, 30.0), ks=(0.01, -0.5, 3.0, -20.0), slice_mult=2),
+           W.quad(0.6, -0.33, slice_mult=4), W.thin_multipole((0.001, -0.3, 2.0, 10.0), (0.002, 0.2, -1.0, 5.0)),
+           W.marker(), W.drift(0.9), W.sbend(1.8, ang, eta=1.002),
+           W.cavity(2e6, 8.0, math.asin(0.2) if ramp else 0.0, +1.0), W.drift(0.5),
+           W.snake(2.0, math.radians(-30))]
+    return W.lattice(els * 3)
+
+
+# ---------------------------------------------------------------------------------------------
+# config 1 (full) and config 2
+# ---------------------------------------------------------------------------------------------
+def test_config1_one_turn_and_ten_turns(gst, O):
+    c = W.config(1)
+    for turns, tol in ((1, 1e-12), (10, 1e-11)):
+        ref, rlost, _ = O.track(c["lattice"], c["beam"], c["state"], turns, c["split"], c["n_slices"], c["depth"])
+        got, lost, pol, emit, _ = gpu_track(gst, c["lattice"], c["beam"], c["state"], turns, c["split"], c["n_slices"], c["depth"])
+        assert not rlost.any() and not lost.any()
+        assert orbit_err(got, ref) < tol, (turns, orbit_err(got, ref))
+        assert spin_err(got, ref) < tol, (turns, spin_err(got, ref))
+        rp, _ = O.polarization(ref)
+        assert np.max(np.abs(pol - rp)) < 1e-13
+        assert np.max(np.abs(emit / O.emittance(ref) - 1)) < 1e-11
+
+
+def test_config2_one_turn_full_bunch(gst, O):
+    c = W.config(2)
+    ref, rlost, _ = O.track(c["lattice"], c["beam"], c["state"], 1, c["split"], c["n_slices"], c["depth"])
+    got, lost, pol, emit, _ = gpu_track(gst, c["lattice"], c["beam"], c["state"], 1, c["split"], c["n_slices"], c["depth"])
+    assert not rlost.any() and not lost.any()
+    assert orbit_err(got, ref) < 1e-12, orbit_err(got, ref)
+    assert spin_err(got, ref) < 1e-12, spin_err(got, ref)
+
+
+def test_config2_hundred_turns(gst, O):
+    c = W.config(2, n_particles=192)
+    ref, rlost, _ = O.track(c["lattice"], c["beam"], c["state"], 100, c["split"], c["n_slices"], c["depth"])
+    got, lost, pol, emit, _ = gpu_track(gst, c["lattice"], c["beam"], c["state"], 100, c["split"], c["n_slices"], c["depth"])
+    assert not rlost.any() and not lost.any()
+    assert orbit_err(got, ref) < 1e-9, orbit_err(got, ref)
+    assert spin_err(got, ref) < 1e-9, spin_err(got, ref)
+
+
+# ---------------------------------------------------------------------------------------------
+# every split x depth on a lattice with every element type; ragged particle count
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("split", [W.SPLIT_DRIFT_KICK, W.SPLIT_BEND_KICK, W.SPLIT_MATRIX_KICK])
+@pytest.mark.parametrize("depth,n_slices", [(1, 1), (1, 3), (2, 2), (3, 4), (4, 8), (5, 16), (6, 32)])
+def test_all_splits_depths_all_element_types(gst, O, split, depth, n_slices):
+    lat = mixed_lattice()
+    bm = W.beam(12.0)
+    n = 200                                   # 3 full blocks of 64 and a ragged tail of 8
+    st = W.gaussian_bunch(7, n, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
+    ref, rlost, g_ref = O.track(lat, bm, st, 2, split, n_slices, depth)
+    got, lost, pol, emit, g_gpu = gpu_track(gst, lat, bm, st, 2, split, n_slices, depth)
+    assert not rlost.any() and not lost.any()
+    assert orbit_err(got, ref) < 2e-12, orbit_err(got, ref)
+    assert spin_err(got, ref) < 2e-12, spin_err(got, ref)
+    assert abs(g_gpu - g_ref) < 1e-12 * g_ref
+    assert np.max(np.abs(np.linalg.norm(got[6:9], axis=0) - 1)) < 1e-12     # A9: |S| = 1 without renormalising
+
+
+def test_large_angle_per_slice_takes_the_sincos_branch(gst, O):
+    # one slice through a strong bend at high G*gamma: rotation angle per edge > 1.4 rad
+    lat = W.lattice([W.sbend(9.45, 0.2), W.drift(1.0)])
+    bm = W.beam(W.gamma_for_Ggamma(45.5))
+    st = W.gaussian_bunch(3, 70, bm["gamma0"], 1e-3, 1e-4, 1e-3, 1e-4, 1e-4, 0.0, "sphere")
+    ref, _, _ = O.track(lat, bm, st, 1, W.SPLIT_BEND_KICK, 1, 1)
+    got, lost, *_ = gpu_track(gst, lat, bm, st, 1, W.SPLIT_BEND_KICK, 1, 1)
+    assert spin_err(got, ref) < 1e-12 and orbit_err(got, ref) < 1e-12
+
+
+# ---------------------------------------------------------------------------------------------
+# edge cases
+# ---------------------------------------------------------------------------------------------
+def test_empty_and_single_particle_bunches(gst, O):
+    c = W.config(1)
+    L = gst.Lattice(c["lattice"], c["beam"])
+    d0 = torch.zeros((9, 0), dtype=torch.float64, device="cuda")
+    b0 = gst.Bunch(d0)
+    b0.track(L, 3, c["split"], 4, 3)
+    pol, nl = b0.polarization()
+    assert nl == 0 and np.all(pol == 0)
+    b0.close()
+    st = c["state"][:, :1].copy()
+    ref, _, _ = O.track(c["lattice"], c["beam"], st, 3, c["split"], 4, 3)
+    got, lost, *_ = gpu_track(gst, c["lattice"], c["beam"], st, 3, c["split"], 4, 3)
+    assert orbit_err(got, ref) < 1e-12 and spin_err(got, ref) < 1e-12
+    L.close()
+
+
+def test_invalid_arguments_are_rejected(gst):
+    c = W.config(1)
+    L = gst.Lattice(c["lattice"], c["beam"])
+    d = torch.tensor(c["state"], dtype=torch.float64, device="cuda")
+    b = gst.Bunch(d)
+    for args in ((1, 1, 4, 0), (1, 1, 4, 7), (1, 1, 0, 1), (1, 3, 4, 1), (1, 1, 4, 4), (-1, 1, 4, 1)):
+        with pytest.raises(gst.GstError) as ei:
+            b.track(L, *args)
+        assert ei.value.status == gst.EINVAL
+    bad = c["lattice"].copy()
+    bad[1]["kn"][0] = 0.0
+    with pytest.raises(gst.GstError):
+        gst.Lattice(bad, c["beam"])
+    bad = c["lattice"].copy()
+    bad[3]["h"] = 0.0
+    with pytest.raises(gst.GstError):
+        gst.Lattice(bad, c["beam"])
+    bad = c["lattice"].copy()
+    bad[0]["type"] = 11
+    with pytest.raises(gst.GstError):
+        gst.Lattice(bad, c["beam"])
+    b.close()
+    L.close()
+
+
+def test_lost_particles_are_flagged_identically_and_excluded_from_reductions(gst, O):
+    c = W.config(1)
+    st = c["state"].copy()
+    st[1, 5] = 1.5          # |Px| > P: square root of a negative number in the first element (A15)
+    st[3, 17] = -2.0
+    ref, rlost, _ = O.track(c["lattice"], c["beam"], st, 2, c["split"], 4, 3)
+    got, lost, pol, emit, _ = gpu_track(gst, c["lattice"], c["beam"], st, 2, c["split"], 4, 3)
+    assert rlost[5] and rlost[17]
+    assert np.array_equal(lost.astype(bool), rlost.astype(bool))
+    keep = ~rlost.astype(bool)
+    assert orbit_err(got[:, keep], ref[:, keep]) < 1e-12
+    rp, nl = O.polarization(ref, rlost)
+    assert np.max(np.abs(pol - rp)) < 1e-13
+    assert np.max(np.abs(emit / O.emittance(ref, rlost) - 1)) < 1e-11
+
+
+def test_chunked_tracking_is_bit_identical_to_one_call(gst):
+    lat = mixed_lattice(ramp=True)
+    bm = W.beam(12.0)
+    st = W.gaussian_bunch(9, 130, 12.0, 1e-3, 1e-4, 1e-3, 1e-4, 3e-4, 0.05, "sphere")
+    a, *_ , ga = gpu_track(gst, lat, bm, st, 12, W.SPLIT_MATRIX_KICK, 4, 3)
+    b, *_ , gb = gpu_track(gst, lat, bm, st, 12, W.SPLIT_MATRIX_KICK, 4, 3, chunks=[5, 4, 3])
+    assert np.array_equal(a, b) and ga == gb
+
+
+def test_host_buffer_entry_point_matches_device_path(gst):
+    c = W.config(1)
+    dev, lost, pol, *_ = gpu_track(gst, c["lattice"], c["beam"], c["state"], 4, c["split"], 4, 3)
+    L = gst.Lattice(c["lattice"], c["beam"])
+    host = [np.ascontiguousarray(c["state"][i]) for i in range(9)]
+    hpol, nl = L.track_host(host, 4, c["split"], 4, 3)
+    assert np.array_equal(np.stack(host), dev) and np.array_equal(hpol, pol) and nl == 0
+    L.close()
+
+
+def test_reductions_match_oracle_on_a_large_bunch(gst, O):
+    rng = np.random.default_rng(12)
+    n = 300_001
+    st = rng.normal(size=(9, n)) * np.array([1e-3, 1e-4, 2e-3, 3e-4, 0.1, 1e-3, 1, 1, 1])[:, None]
+    st[0] += 5e-3           # offset beam: the mean-subtracted second pass must handle it
+    d = torch.tensor(st, dtype=torch.float64, device="cuda").contiguous()
+    b = gst.Bunch(d)
+    pol, nl = b.polarization()
+    emit = b.emittance()
+    rp, _ = O.polarization(st)
+    assert nl == 0 and np.max(np.abs(pol - rp)) < 1e-14
+    assert np.max(np.abs(emit / O.emittance(st) - 1)) < 1e-12
+    b.close()
+
+
+# ---------------------------------------------------------------------------------------------
+# RHIC-like ring (configs 3, 4, 5): reduced sizes in full, full size on sampled particles
+# ---------------------------------------------------------------------------------------------
+def test_config3_reduced_per_particle_and_polarization(gst, O):
+    c = W.config(3, n_particles=512)
+    ref, rlost, _ = O.track(c["lattice"], c["beam"], c["state"], 20, c["split"], c["n_slices"], c["depth"])
+    got, lost, pol, emit, _ = gpu_track(gst, c["lattice"], c["beam"], c["state"], 20, c["split"], c["n_slices"], c["depth"])
+    assert not rlost.any() and not lost.any()
+    assert orbit_err(got, ref) < 1e-10 and spin_err(got, ref) < 1e-10, (orbit_err(got, ref), spin_err(got, ref))
+    rp, _ = O.polarization(ref)
+    assert np.max(np.abs(pol - rp)) < 1e-9
+
+
+def test_config4_ramp_reduced(gst, O):
+    c = W.config(4, n_particles=256)
+    ref, rlost, g_ref = O.track(c["lattice"], c["beam"], c["state"], 40, c["split"], c["n_slices"], c["depth"])
+    got, lost, pol, emit, g_gpu = gpu_track(gst, c["lattice"], c["beam"], c["state"], 40, c["split"], c["n_slices"],
+                                            c["depth"], chunks=[10, 10, 10, 10])
+    assert not rlost.any() and not lost.any()
+    assert abs(g_gpu - g_ref) < 1e-13 * g_ref
+    assert abs(W.G_PROTON * (g_gpu - c["beam"]["gamma0"]) - 40 * 1.9108e-4) < 1e-6      # A13
+    assert orbit_err(got, ref) < 1e-10 and spin_err(got, ref) < 1e-10, (orbit_err(got, ref), spin_err(got, ref))
+    rp, _ = O.polarization(ref)
+    assert np.max(np.abs(pol - rp)) < 1e-6
+
+
+@pytest.mark.parametrize("split", [W.SPLIT_DRIFT_KICK, W.SPLIT_BEND_KICK, W.SPLIT_MATRIX_KICK])
+def test_config5_sweep_points_reduced(gst, O, split):
+    c = W.config(5, n_particles=128)
+    for n_slices, depth in ((1, 1), (4, 3), (16, 5)):
+        ref, rlost, _ = O.track(c["lattice"], c["beam"], c["state"], 3, split, n_slices, depth)
+        got, lost, pol, *_ = gpu_track(gst, c["lattice"], c["beam"], c["state"], 3, split, n_slices, depth)
+        assert not rlost.any() and not lost.any()
+        assert orbit_err(got, ref) < 1e-11 and spin_err(got, ref) < 1e-11, (n_slices, depth, orbit_err(got, ref), spin_err(got, ref))
+        rp, _ = O.polarization(ref)
+        assert np.max(np.abs(pol - rp)) < 1e-6
+
+
+def test_config3_full_size_sampled_particles(gst, O):
+    """65536 particles x 1000 turns in the launch configuration bench.py times; the oracle tracks a
+    sample of the same particles one by one (particles are independent)."""
+    c = W.config(3)
+    n = c["state"].shape[1]
+    assert n == 65536 and c["n_turns"] == 1000
+    got, lost, pol, emit, _ = gpu_track(gst, c["lattice"], c["beam"], c["state"], 1000, c["split"], c["n_slices"], c["depth"])
+    assert not lost.any()
+    idx = np.array([0, 63, 64, 4097, 20000, 32767, 50001, 65535])      # several blocks, first and last lanes
+    ref, rlost, _ = O.track(c["lattice"], c["beam"], c["state"][:, idx], 1000, c["split"], c["n_slices"], c["depth"])
+    assert not rlost.any()
+    sub = got[:, idx]
+    assert orbit_err(sub, ref) < 1e-8 and spin_err(sub, ref) < 1e-8, (orbit_err(sub, ref), spin_err(sub, ref))
+    rp, _ = O.polarization(ref)
+    sp = sub[6:9].mean(axis=1)
+    assert np.max(np.abs(sp - rp[:3])) < 1e-6                           # north_star: polarization within 1e-6
+    # properties that hold at any size: unit spins, snakes keep the bunch polarized near the vertical
+    assert np.max(np.abs(np.linalg.norm(got[6:9], axis=0) - 1)) < 1e-11
+    assert abs(pol[3] - np.linalg.norm(got[6:9].mean(axis=1))) < 1e-12
