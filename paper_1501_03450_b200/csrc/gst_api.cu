@@ -86,6 +86,7 @@ gst::DevElem derive(const gst_element& e, int n_slices, double C) {
     d.ks[m - 2] = e.ks[m - 2];
     if (e.kn[m - 2] != 0.0 || e.ks[m - 2] != 0.0) d.order = m;
   }
+  d.pure_quad = (d.order == 2 && e.ks[0] == 0.0) ? 1 : 0;
   if (e.type == GST_SBEND) {
     long double h = e.h, k0 = e.k0, ds = (long double)e.L / d.N;
     long double half = sinl(0.5L * h * ds);

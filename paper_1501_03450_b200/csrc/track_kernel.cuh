@@ -9,6 +9,13 @@
 // The orbit maps are algebraically equal to the paper's formulas (10), (24), (25), (29), (31) but
 // are written in cancellation-free form: the literal forms subtract O(1)
 // quantities to get O(1e-3) results, which costs ~1e-11 of the bunch scale per slice in fp64.
+//
+// Scheduling: the kernel runs at ~3.5 warps per SM sub-partition, so the FP64
+// pipe is fed by instruction-level parallelism inside a thread.  The slice loop is software
+// pipelined -- orbit slice i+1 is independent of the quaternion work of edge i and sits in the same
+// basic block -- and the loop body is branch-free: reciprocal and reciprocal square root are
+// MUFU seeds + Newton steps without slow-path calls, domain errors set a sticky flag, and the
+// Romberg-level membership of an edge is resolved at compile time for odd edges.
 #pragma once
 #include <cstdint>
 
@@ -21,8 +28,8 @@ enum : int { SPLIT_DK = 0, SPLIT_BK = 1, SPLIT_MK = 2 };
 struct __align__(16) DevElem {
   int type;
   int N;          // slices of this element (thick), else 1
-  int order;      // highest multipole order present (2..5), 0 if none
-  int pad;
+  int order;      // highest multipole order present (2..5); 2 if none
+  int pure_quad;  // 1 when only kn[0] is non-zero
   double L;       // length
   double ds;      // L / N
   double h, k0;
@@ -62,6 +69,31 @@ struct TrackArgs {
 };
 
 struct Quat { double w, x, y, s; };
+
+// ---------------------------------------------------------------------------------------------
+// branch-free reciprocal and reciprocal square root: 20-bit MUFU seed + Newton in FMAs.
+// (CUDA's 1.0/x and sqrt() carry a slow-path call that splits the basic block.)
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ double rcp_nr(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x, y, 1.0);
+  e = fma(e, e, e);                 // e + e^2: one cubic step  y (1 + e + e^2)
+  y = fma(y, e, y);                 // relative error ~2^-60
+  e = fma(-x, y, 1.0);
+  return fma(y, e, y);              // polish to ~1 ulp
+}
+__device__ __forceinline__ double rsqrt_nr(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double t = x * y;
+  double e = fma(-t, y, 1.0);       // 1 - x y^2
+  double c = fma(0.375, e, 0.5);
+  y = fma(y * e, c, y);             // cubic step, relative error ~2^-58
+  t = x * y;
+  e = fma(-t, y, 1.0);
+  return fma(0.5 * y, e, y);        // polish to ~1 ulp
+}
 
 // reference-particle and per-particle constants that change only when Pt or E0 changes
 struct Ref {
@@ -103,44 +135,49 @@ __device__ __forceinline__ void pcon_set(PCon& c, double Pt, const Ref& r, doubl
 // ---------------------------------------------------------------------------------------------
 // quaternions (a10, a11)
 // ---------------------------------------------------------------------------------------------
-// q = (cos(th/2), sin(th/2) w/th) for rotation vector w: both factors are even in th, so for
-// th^2/4 <= 0.5 they are polynomials in th^2 -- no sqrt, no division, no sincos ("low-order
-// polynomials", here taken to full double precision).
+// q = (cos(th/2), sin(th/2) w/th) for rotation vector w: both factors are even in th, so they are
+// power series in v = th^2 -- no sqrt, no division, no sincos ("low-order polynomials", here
+// taken to full double precision).  Three tiers by angle; the first is the straight-line path.
 __device__ __forceinline__ Quat quat_from_rotvec(double wx, double wy, double ws) {
-  double t2 = fma(wx, wx, fma(wy, wy, ws * ws));
-  double u = 0.25 * t2;   // (th/2)^2
-  Quat q;
-  if (u <= 0.5) {
-    // cos x = sum (-u)^k/(2k)!,  sin x / x = sum (-u)^k/(2k+1)!,  k = 0..9  (remainder < 4e-20)
-    double c = -1.0 / 6402373705728000.0;        // 1/18!
-    double s = -1.0 / 121645100408832000.0;      // 1/19!
-    c = fma(c, u, 1.0 / 20922789888000.0);       // 16!
-    s = fma(s, u, 1.0 / 355687428096000.0);      // 17!
-    c = fma(c, u, -1.0 / 87178291200.0);         // 14!
-    s = fma(s, u, -1.0 / 1307674368000.0);       // 15!
-    c = fma(c, u, 1.0 / 479001600.0);            // 12!
-    s = fma(s, u, 1.0 / 6227020800.0);           // 13!
-    c = fma(c, u, -1.0 / 3628800.0);             // 10!
-    s = fma(s, u, -1.0 / 39916800.0);            // 11!
-    c = fma(c, u, 1.0 / 40320.0);                // 8!
-    s = fma(s, u, 1.0 / 362880.0);               // 9!
-    c = fma(c, u, -1.0 / 720.0);                 // 6!
-    s = fma(s, u, -1.0 / 5040.0);                // 7!
-    c = fma(c, u, 1.0 / 24.0);
-    s = fma(s, u, 1.0 / 120.0);
-    c = fma(c, u, -0.5);
-    s = fma(s, u, -1.0 / 6.0);
-    c = fma(c, u, 1.0);
-    s = fma(s, u, 1.0);
-    s *= 0.5;                                    // sin(th/2)/th = (1/2) sin(x)/x
-    q.w = c; q.x = s * wx; q.y = s * wy; q.s = s * ws;
-  } else {
-    double th = sqrt(t2), sn, cs;
-    sincos(0.5 * th, &sn, &cs);
-    double f = sn / th;
-    q.w = cs; q.x = f * wx; q.y = f * wy; q.s = f * ws;
+  const double v = fma(wx, wx, fma(wy, wy, ws * ws));   // th^2;  x = th/2, x^2 = v/4
+  // tier 1: v <= 0.5 (th <= 0.707): cos x = sum_k (-v/4)^k/(2k)!, sin(x)/th = (1/2) sum_k (-v/4)^k/(2k+1)!,
+  // k = 0..6, remainder (v/4)^7/14! < 6e-18
+  double c = 1.0 / (4096.0 * 479001600.0);              // + (v/4)^6/12!
+  double s = 0.5 / (4096.0 * 6227020800.0);             // + (1/2)(v/4)^6/13!
+  c = fma(c, v, -1.0 / (1024.0 * 3628800.0));
+  s = fma(s, v, -0.5 / (1024.0 * 39916800.0));
+  c = fma(c, v, 1.0 / (256.0 * 40320.0));
+  s = fma(s, v, 0.5 / (256.0 * 362880.0));
+  c = fma(c, v, -1.0 / (64.0 * 720.0));
+  s = fma(s, v, -0.5 / (64.0 * 5040.0));
+  c = fma(c, v, 1.0 / (16.0 * 24.0));
+  s = fma(s, v, 0.5 / (16.0 * 120.0));
+  c = fma(c, v, -1.0 / 8.0);
+  s = fma(s, v, -0.5 / 24.0);
+  c = fma(c, v, 1.0);
+  s = fma(s, v, 0.5);
+  if (__builtin_expect(v > 0.5, 0)) {
+    if (v <= 2.0) {
+      // tier 2: u = v/4 <= 0.5, k = 0..9, remainder < 4e-20
+      double u = 0.25 * v;
+      c = -1.0 / 6402373705728000.0;  s = -1.0 / 121645100408832000.0;
+      c = fma(c, u, 1.0 / 20922789888000.0);  s = fma(s, u, 1.0 / 355687428096000.0);
+      c = fma(c, u, -1.0 / 87178291200.0);    s = fma(s, u, -1.0 / 1307674368000.0);
+      c = fma(c, u, 1.0 / 479001600.0);       s = fma(s, u, 1.0 / 6227020800.0);
+      c = fma(c, u, -1.0 / 3628800.0);        s = fma(s, u, -1.0 / 39916800.0);
+      c = fma(c, u, 1.0 / 40320.0);           s = fma(s, u, 1.0 / 362880.0);
+      c = fma(c, u, -1.0 / 720.0);            s = fma(s, u, -1.0 / 5040.0);
+      c = fma(c, u, 1.0 / 24.0);              s = fma(s, u, 1.0 / 120.0);
+      c = fma(c, u, -0.5);                    s = fma(s, u, -1.0 / 6.0);
+      c = fma(c, u, 1.0);                     s = fma(s, u, 1.0);
+      s *= 0.5;
+    } else {
+      double th = sqrt(v), sn, cs;
+      sincos(0.5 * th, &sn, &cs);
+      c = cs; s = sn / th;
+    }
   }
-  return q;
+  return Quat{c, s * wx, s * wy, s * ws};
 }
 // a (x) b
 __device__ __forceinline__ Quat quat_mul(const Quat& a, const Quat& b) {
@@ -175,16 +212,26 @@ template <int DEPTH> struct SpinAcc {
 #pragma unroll
     for (int l = 0; l < DEPTH; ++l) Q[l] = Quat{1.0, 0.0, 0.0, 0.0};
   }
-  // (wx,wy,ws) = weight * ds * Omega_i with weight 1/2 at the two ends of the element
-  __device__ __forceinline__ void edge(int i, double wx, double wy, double ws) {
+  // fold rotation vector (weight * ds * Omega_i) into levels 0..NS-1, all known at compile time
+  template <int NS>
+  __device__ __forceinline__ Quat fold_static(double wx, double wy, double ws) {
     Quat q = quat_from_rotvec(wx, wy, ws);
     Q[0] = quat_mul(q, Q[0]);
 #pragma unroll
-    for (int l = 1; l < DEPTH; ++l) {
-      if ((i & ((1 << l) - 1)) == 0) {
-        q = quat_double(q);
-        Q[l] = quat_mul(q, Q[l]);
-      }
+    for (int l = 1; l < NS; ++l) {
+      q = quat_double(q);
+      Q[l] = quat_mul(q, Q[l]);
+    }
+    return q;
+  }
+  // continue from level FROM upwards while 2^l | i (run-time, uniform across the grid)
+  template <int FROM>
+  __device__ __forceinline__ void fold_dynamic(int i, Quat q) {
+#pragma unroll
+    for (int l = FROM; l < DEPTH; ++l) {
+      if ((i & ((1 << l) - 1)) != 0) return;
+      q = quat_double(q);
+      Q[l] = quat_mul(q, Q[l]);
     }
   }
   // Romberg limit (39b) P:542 of the level products, normalised, applied to S (a11)
@@ -205,7 +252,7 @@ template <int DEPTH> struct SpinAcc {
     }
     Quat q = Q[0];
     double n2 = fma(q.w, q.w, fma(q.x, q.x, fma(q.y, q.y, q.s * q.s)));
-    double rn = rsqrt(n2);
+    double rn = rsqrt_nr(n2);
     q.w *= rn; q.x *= rn; q.y *= rn; q.s *= rn;
     quat_rotate(q, Sx, Sy, Ss);
   }
@@ -224,16 +271,185 @@ __device__ __forceinline__ bool drift(State& z, double L, const PCon& c, const R
   double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
   double ps2m1 = c.e0 - pt2;
   double ps2 = 1.0 + ps2m1;
-  if (!(ps2 > 0.0)) return false;
-  double Ps = sqrt(ps2);
-  double rr = 1.0 / (Ps * (Ps + 1.0));
-  double iPs = rr * (Ps + 1.0), iPs1 = rr * Ps;
+  double iPs = rsqrt_nr(ps2);
+  double Ps = ps2 * iPs;
+  double iPs1 = rcp_nr(Ps + 1.0);
   double LiPs = L * iPs;
   z.X = fma(LiPs, z.Px, z.X);
   z.Y = fma(LiPs, z.Py, z.Y);
-  double num = (c.tA - pt2 * r.ibeta0 - z.Pt * ps2m1 * iPs1) * iPs1;
+  double num = (fma(-pt2, r.ibeta0, c.tA) - z.Pt * ps2m1 * iPs1) * iPs1;
   z.T = fma(LiPs, num, z.T);
-  return true;
+  return ps2 > 0.0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// thick elements: a "stepper" advances the orbit by one slice and evaluates weight*ds*Omega at the
+// current point; run_thick drives it through the N slices with the spin work software-pipelined.
+// ---------------------------------------------------------------------------------------------
+template <int DEPTH, class Stepper>
+__device__ __forceinline__ void run_thick(Stepper& s, int N, double ds, double& Sx, double& Sy, double& Ss) {
+  SpinAcc<DEPTH> acc;
+  acc.reset();
+  const double hds = 0.5 * ds;
+  double wx, wy, ws;
+  s.omega(hds, wx, wy, ws);                       // pending edge 0, half weight
+  if (DEPTH == 1) {
+    for (int i = 1; i <= N; ++i) {
+      s.advance();                                // orbit slice i ...
+      acc.template fold_static<1>(wx, wy, ws);    // ... independent of the spin work of edge i-1
+      s.omega(i == N ? hds : ds, wx, wy, ws);
+    }
+    acc.template fold_static<1>(wx, wy, ws);
+  } else {
+    // DEPTH >= 2: N is even (A4).  Edges are taken in pairs (even, odd): the odd edge belongs to
+    // level 0 only, the even edge to levels 0 and 1 and, where 4 | i, 8 | i, ..., to higher ones.
+    for (int i = 0; i < N; i += 2) {
+      s.advance();
+      {
+        Quat q = acc.template fold_static<2>(wx, wy, ws);    // even edge i
+        acc.template fold_dynamic<2>(i, q);
+      }
+      s.omega(ds, wx, wy, ws);
+      s.advance();
+      acc.template fold_static<1>(wx, wy, ws);               // odd edge i+1
+      s.omega(i + 2 == N ? hds : ds, wx, wy, ws);
+    }
+    acc.template fold_static<DEPTH>(wx, wy, ws);             // edge N: every level (2^(DEPTH-1) | N)
+  }
+  acc.finish(Sx, Sy, Ss);
+}
+
+// a4: exact sector bend (10), spin from the slice-edge Omega (6b).
+// With c = cos(h ds), s = sin(h ds), A = sqrt(Pa^2 - Px^2), g = A - eta(1 + hX):
+//   Px_f = Px + [g s - Px (1-c)]                                                    (10b)
+//   X_f  = X + g (ck - sk r) + Px (sk + ck r),  r = (Px + Px_f)/(A + A_f)           (10a) rearranged
+// Y and T do not feed back into the motion or Omega, so they are advanced once per element from
+// the total asin difference (group property of the flow).
+struct BendExact {
+  double &X, &Px;
+  double A, Am1, iA;
+  double Pa2, q2, a1k;
+  double h, k0, cm, sn, ck, sk, ome;
+  bool bad;
+  __device__ __forceinline__ BendExact(State& z, const DevElem& e, const PCon& c)
+      : X(z.X), Px(z.Px), h(e.h), k0(e.k0), cm(e.cm), sn(e.sn), ck(e.ck), sk(e.sk), ome(e.ome) {
+    const double ea = fma(-z.Py, z.Py, c.e0);     // Pa^2 - 1                                  (8)
+    Pa2 = 1.0 + ea;
+    const double a2 = fma(-z.Px, z.Px, Pa2);
+    bad = !(a2 > 0.0);
+    iA = rsqrt_nr(a2);
+    A = a2 * iA;
+    Am1 = fma(-z.Px, z.Px, ea) * rcp_nr(A + 1.0);  // A - 1 without cancellation
+    q2 = c.a2p * e.k0 * z.Py;                      // G(gamma-1) (u.b) / P  per unit momentum component
+    a1k = fma(c.a1, e.k0, -q2 * z.Py);
+  }
+  __device__ __forceinline__ void advance() {
+    const double g = (Am1 + ome) - k0 * X;
+    const double dPx = fma(g, sn, -Px * cm);
+    const double Pxf = Px + dPx;
+    const double f2 = fma(-Pxf, Pxf, Pa2);
+    bad |= !(f2 > 0.0);
+    const double y = rsqrt_nr(f2);
+    const double Af = f2 * y;
+    const double rr = (Px + Pxf) * rcp_nr(Af + A);
+    X = fma(g, fma(-sk, rr, ck), fma(Px, fma(ck, rr, sk), X));
+    Am1 = fma(-dPx, rr, Am1);
+    Px = Pxf; A = Af; iA = y;
+  }
+  // Omega = -(1+hX)/Ps [a1 b - a2 (u.b) u] + h y-hat with b = (0, k0, 0), Ps = A
+  __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) const {
+    const double fw = fma(h, X, 1.0) * iA * w;
+    const double fq = fw * q2;
+    wx = fq * Px;
+    wy = fma(-fw, a1k, w * h);
+    ws = fq * A;
+  }
+};
+
+template <int DEPTH>
+__device__ __forceinline__ bool sbend_exact(State& z, const DevElem& e, const PCon& c, const Ref& r) {
+  BendExact s(z, e, c);
+  const double A0 = s.A, Am1_0 = s.Am1, Px0 = z.Px;
+  run_thick<DEPTH>(s, e.N, e.ds, z.Sx, z.Sy, z.Ss);
+  // asin(Px0/Pa) - asin(PxN/Pa) = asin(x),  x = (Px0 A_N - Px_N A_0)/Pa^2  (no cancellation)
+  const double x = fma(Px0, s.Am1 - Am1_0, -(z.Px - Px0) * A0) * rcp_nr(s.Pa2);
+  const double v = x * x;
+  double dasin;
+  if (v < 2.5e-3) {     // asin(x)/x = 1 + v/6 + 3v^2/40 + 15v^3/336 + 105v^4/3456 + 945v^5/42240 + 10395v^6/599040
+    double p = 10395.0 / 599040.0;
+    p = fma(p, v, 945.0 / 42240.0);
+    p = fma(p, v, 105.0 / 3456.0);
+    p = fma(p, v, 15.0 / 336.0);
+    p = fma(p, v, 3.0 / 40.0);
+    p = fma(p, v, 1.0 / 6.0);
+    dasin = fma(p * v, x, x);
+  } else {
+    dasin = asin(x);
+  }
+  const double dh = dasin * e.inv_h;
+  z.Y = fma(z.Py * e.inv_eta, e.L + dh, z.Y);
+  z.T += e.inv_eta * (fma(-z.Pt, e.L, -c.ibpt * dh) - e.ome * e.L * r.ibeta0);
+  return !s.bad;
+}
+
+// a5: TEAPOT sector bend (30)(31): half curved drift, kick -ds k0 (1+hX), half curved drift.
+// The curved drift is a straight line seen from the rotating frame, so (Px,Ps) simply rotate by
+// phi = h ds/2; X, Y, T use rho(sec phi - 1), rho tan phi and rho(tan phi - phi) from the host.
+struct BendTeapot {
+  State& z;
+  const DevElem& e;
+  const PCon& c;
+  double Ps, iPs, pa2, q2, a1k, hds;
+  bool bad;
+  __device__ __forceinline__ BendTeapot(State& z_, const DevElem& e_, const PCon& c_) : z(z_), e(e_), c(c_) {
+    pa2 = fma(-z.Py, z.Py, 1.0 + c.e0);
+    const double ps2 = fma(-z.Px, z.Px, pa2);
+    bad = !(ps2 > 0.0);
+    iPs = rsqrt_nr(ps2);
+    Ps = ps2 * iPs;
+    q2 = c.a2p * e.k0 * z.Py;
+    a1k = fma(c.a1, e.k0, -q2 * z.Py);
+    hds = 0.5 * e.ds;
+  }
+  __device__ __forceinline__ void half_drift() {
+    const double xp = z.Px * iPs;
+    const double D = fma(-xp, e.ht, 1.0);
+    bad |= !(D > 0.0);
+    const double iD = rcp_nr(D);
+    // delta q = [(rho+X) tan phi - s Ps D]/(Ps D),  s = ds/2
+    const double num = e.r_tanmphi + fma(z.X, e.ht, hds * fma(z.Px, e.ht, -(Ps - 1.0)));
+    const double dq = num * iPs * iD;
+    z.X = (e.r_secm1 + fma(z.X, e.hsec, e.r_tan * xp)) * iD;
+    z.Y = fma(z.Py, hds + dq, z.Y);
+    z.T += fma(-z.Pt, hds, -c.ibpt * dq);
+    const double Pxn = fma(z.Px, e.hc, Ps * e.hs);
+    Ps = fma(Ps, e.hc, -z.Px * e.hs);
+    z.Px = Pxn;
+    bad |= !(Ps > 0.0);
+  }
+  __device__ __forceinline__ void advance() {
+    iPs = rcp_nr(Ps);
+    half_drift();
+    z.Px = fma(-e.ds * e.k0, fma(e.h, z.X, 1.0), z.Px);
+    const double ps2 = fma(-z.Px, z.Px, pa2);
+    bad |= !(ps2 > 0.0);
+    iPs = rsqrt_nr(ps2);
+    Ps = ps2 * iPs;
+    half_drift();
+  }
+  __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) const {
+    const double fw = fma(e.h, z.X, 1.0) * rcp_nr(Ps) * w;
+    const double fq = fw * q2;
+    wx = fq * z.Px;
+    wy = fma(-fw, a1k, w * e.h);
+    ws = fq * Ps;
+  }
+};
+template <int DEPTH>
+__device__ __forceinline__ bool sbend_teapot(State& z, const DevElem& e, const PCon& c) {
+  BendTeapot s(z, e, c);
+  run_thick<DEPTH>(s, e.N, e.ds, z.Sx, z.Sy, z.Ss);
+  return !s.bad;
 }
 
 // multipole field (28): By + i Bx = sum_m (kn_m + i ks_m)(X+iY)^(m-1), Horner from the top order
@@ -249,175 +465,94 @@ __device__ __forceinline__ void mult_field(const DevElem& e, double X, double Y,
   bx = fma(re, Y, im * X);
 }
 
-// a9 for straight elements (h = 0):  Omega = -(1/Ps)[a1 b - a2 (u.b) u],  b = (bx, by, 0)
-__device__ __forceinline__ void omega_straight(double Px, double Py, double iPs, double bx, double by, const PCon& c,
-                                               double& ox, double& oy, double& os) {
-  double pb = c.a2p * fma(Px, bx, Py * by);
-  ox = -iPs * fma(c.a1, bx, -pb * Px);
-  oy = -iPs * fma(c.a1, by, -pb * Py);
-  os = pb;
-}
-
-// ---------------------------------------------------------------------------------------------
-// thick elements
-// ---------------------------------------------------------------------------------------------
-
-// a4: exact sector bend (10) in N slices, spin from the slice-edge Omega (6b).
-// With c = cos(h ds), s = sin(h ds), A = sqrt(Pa^2 - Px^2), g = A - eta(1 + hX):
-//   Px_f = Px + [g s - Px (1-c)]                                                    (10b)
-//   X_f  = X + g (ck - sk r) + Px (sk + ck r),  r = (Px + Px_f)/(A + A_f)           (10a) rearranged
-// Y and T do not feed back into the motion or Omega, so they are advanced once per element from
-// the total asin difference (group property of the flow).
-template <int DEPTH>
-__device__ __forceinline__ bool sbend_exact(State& z, const DevElem& e, const PCon& c, const Ref& r) {
-  const double ea = fma(-z.Py, z.Py, c.e0);   // Pa^2 - 1                                  (8)
-  const double Pa2 = 1.0 + ea;
-  double a2 = fma(-z.Px, z.Px, Pa2);
-  if (!(a2 > 0.0)) return false;
-  double A = sqrt(a2);
-  double Am1 = fma(-z.Px, z.Px, ea) / (A + 1.0);   // A - 1 without cancellation
-  const double A0 = A, Am1_0 = Am1, Px0 = z.Px;
-  const double q2 = c.a2p * e.k0 * z.Py;           // G(gamma-1) (u.b)/P  /  (Py... ) see Omega below
-  const double a1k = c.a1 * e.k0 - q2 * z.Py;
-  SpinAcc<DEPTH> acc;
-  acc.reset();
-  const int N = e.N;
-  const double ds = e.ds;
-  {
-    double f = fma(e.h, z.X, 1.0) / A;
-    double w = 0.5 * ds;
-    acc.edge(0, w * (f * q2 * z.Px), w * (e.h - f * a1k), w * (f * q2 * A));
-  }
-  for (int i = 1; i <= N; ++i) {
-    double g = (Am1 + e.ome) - e.k0 * z.X;
-    double dPx = fma(g, e.sn, -z.Px * e.cm);
-    double Pxf = z.Px + dPx;
-    double f2 = fma(-Pxf, Pxf, Pa2);
-    if (!(f2 > 0.0)) return false;
-    double Af = sqrt(f2);
-    double t = 1.0 / (Af * (Af + A));
-    double iAf = t * (Af + A);
-    double rr = (z.Px + Pxf) * (t * Af);
-    z.X += fma(g, fma(-e.sk, rr, e.ck), z.Px * fma(e.ck, rr, e.sk));
-    Am1 = fma(-dPx, rr, Am1);
-    z.Px = Pxf;
-    A = Af;
-    double f = fma(e.h, z.X, 1.0) * iAf;
-    double w = (i == N) ? 0.5 * ds : ds;
-    acc.edge(i, w * (f * q2 * z.Px), w * (e.h - f * a1k), w * (f * q2 * A));
-  }
-  // asin(Px0/Pa) - asin(PxN/Pa) = asin((Px0 A_N - Px_N A_0)/Pa^2)
-  double arg = fma(Px0, Am1 - Am1_0, -(z.Px - Px0) * A0) / Pa2;
-  double dasin = asin(arg);
-  double dh = dasin * e.inv_h;
-  z.Y = fma(z.Py * e.inv_eta, e.L + dh, z.Y);
-  z.T += e.inv_eta * (fma(-z.Pt, e.L, -c.ibpt * dh) - e.ome * e.L * r.ibeta0);
-  acc.finish(z.Sx, z.Sy, z.Ss);
-  return true;
-}
-
-// a5: TEAPOT sector bend (30)(31): half curved drift, kick -ds k0 (1+hX), half curved drift.
-// The curved drift is a straight line seen from the rotating frame, so (Px,Ps) simply rotate by
-// phi = h ds/2; X, Y, T use rho(sec phi - 1), rho tan phi and rho(tan phi - phi) from the host.
-__device__ __forceinline__ bool curved_half_drift(State& z, double& Ps, const DevElem& e, const PCon& c) {
-  double iPs = 1.0 / Ps;
-  double xp = z.Px * iPs;
-  double D = fma(-xp, e.ht, 1.0);
-  if (!(D > 0.0)) return false;
-  double iD = 1.0 / D;
-  double hs2 = 0.5 * e.ds;
-  // delta q = [(rho+X) tan phi - s Ps D]/(Ps D),  s = ds/2
-  double num = e.r_tanmphi + fma(z.X, e.ht, hs2 * fma(z.Px, e.ht, -(Ps - 1.0)));
-  double dq = num * iPs * iD;
-  z.X = (e.r_secm1 + fma(z.X, e.hsec, e.r_tan * xp)) * iD;
-  z.Y = fma(z.Py, hs2 + dq, z.Y);
-  z.T += fma(-z.Pt, hs2, -c.ibpt * dq);
-  double Pxn = fma(z.Px, e.hc, Ps * e.hs);
-  Ps = fma(Ps, e.hc, -z.Px * e.hs);
-  z.Px = Pxn;
-  return Ps > 0.0;
-}
-template <int DEPTH>
-__device__ __forceinline__ bool sbend_teapot(State& z, const DevElem& e, const PCon& c) {
-  const double pa2 = fma(-z.Py, z.Py, 1.0 + c.e0);
-  double ps2 = fma(-z.Px, z.Px, pa2);
-  if (!(ps2 > 0.0)) return false;
-  double Ps = sqrt(ps2);
-  const double q2 = c.a2p * e.k0 * z.Py;
-  const double a1k = c.a1 * e.k0 - q2 * z.Py;
-  SpinAcc<DEPTH> acc;
-  acc.reset();
-  const int N = e.N;
-  const double ds = e.ds;
-  {
-    double f = fma(e.h, z.X, 1.0) / Ps;
-    double w = 0.5 * ds;
-    acc.edge(0, w * (f * q2 * z.Px), w * (e.h - f * a1k), w * (f * q2 * Ps));
-  }
-  for (int i = 1; i <= N; ++i) {
-    if (!curved_half_drift(z, Ps, e, c)) return false;
-    z.Px = fma(-ds * e.k0, fma(e.h, z.X, 1.0), z.Px);
-    ps2 = fma(-z.Px, z.Px, pa2);
-    if (!(ps2 > 0.0)) return false;
-    Ps = sqrt(ps2);
-    if (!curved_half_drift(z, Ps, e, c)) return false;
-    double f = fma(e.h, z.X, 1.0) / Ps;
-    double w = (i == N) ? 0.5 * ds : ds;
-    acc.edge(i, w * (f * q2 * z.Px), w * (e.h - f * a1k), w * (f * q2 * Ps));
-  }
-  acc.finish(z.Sx, z.Sy, z.Ss);
-  return true;
+// a9 for straight elements (h = 0):  w Omega = -(w/Ps)[a1 b - a2 (u.b) u],  b = (bx, by, 0)
+__device__ __forceinline__ void omega_straight(double w, double Px, double Py, double iPs, double bx, double by,
+                                               const PCon& c, double& wx, double& wy, double& ws) {
+  const double pb = c.a2p * fma(Px, bx, Py * by);
+  const double wi = -w * iPs;
+  wx = wi * fma(c.a1, bx, -pb * Px);
+  wy = wi * fma(c.a1, by, -pb * Py);
+  ws = w * pb;
 }
 
 // a7: drift-kick multipole (29): half drift, kick (28), half drift.  The momenta are constant
 // between kicks, so one 1/Ps serves the second half drift, the edge Omega and the next first half.
+// PURE = quadrupole term only (the common case): field and kick collapse to two FMAs.
+template <bool PURE> struct MultDK {
+  State& z;
+  const DevElem& e;
+  const PCon& c;
+  double iPs, tnum, hds, k1, dsk, a1k, ibeta0;
+  bool bad;
+  __device__ __forceinline__ void momenta() {
+    const double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
+    const double ps2m1 = c.e0 - pt2;
+    const double ps2 = 1.0 + ps2m1;
+    bad |= !(ps2 > 0.0);
+    iPs = rsqrt_nr(ps2);
+    const double Ps = ps2 * iPs;
+    const double iPs1 = rcp_nr(Ps + 1.0);
+    tnum = (fma(-pt2, ibeta0, c.tA) - z.Pt * ps2m1 * iPs1) * iPs1 * iPs;   // T' of the drift
+  }
+  __device__ __forceinline__ MultDK(State& z_, const DevElem& e_, const PCon& c_, const Ref& r) : z(z_), e(e_), c(c_) {
+    hds = 0.5 * e.ds;
+    k1 = e.kn[0];
+    dsk = e.ds * k1;
+    a1k = c.a1 * k1;
+    ibeta0 = r.ibeta0;
+    bad = false;
+    momenta();
+  }
+  __device__ __forceinline__ void half_drift() {
+    const double l = hds * iPs;
+    z.X = fma(l, z.Px, z.X);
+    z.Y = fma(l, z.Py, z.Y);
+    z.T = fma(hds, tnum, z.T);
+  }
+  __device__ __forceinline__ void advance() {
+    half_drift();
+    if (PURE) {
+      z.Px = fma(-dsk, z.X, z.Px);
+      z.Py = fma(dsk, z.Y, z.Py);
+    } else {
+      double bx, by;
+      mult_field(e, z.X, z.Y, bx, by);
+      z.Px = fma(-e.ds, by, z.Px);
+      z.Py = fma(e.ds, bx, z.Py);
+    }
+    momenta();
+    half_drift();
+  }
+  __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) const {
+    if (PURE) {
+      const double pb = c.a2p * k1 * (z.Px * z.Y + z.Py * z.X);
+      const double wi = -w * iPs;
+      wx = wi * fma(a1k, z.Y, -pb * z.Px);
+      wy = wi * fma(a1k, z.X, -pb * z.Py);
+      ws = w * pb;
+    } else {
+      double bx, by;
+      mult_field(e, z.X, z.Y, bx, by);
+      omega_straight(w, z.Px, z.Py, iPs, bx, by, c, wx, wy, ws);
+    }
+  }
+};
 template <int DEPTH>
 __device__ __forceinline__ bool mult_dk(State& z, const DevElem& e, const PCon& c, const Ref& r) {
-  SpinAcc<DEPTH> acc;
-  acc.reset();
-  const int N = e.N;
-  const double ds = e.ds, hds = 0.5 * e.ds;
-  double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
-  double ps2m1 = c.e0 - pt2;
-  if (!(1.0 + ps2m1 > 0.0)) return false;
-  double Ps = sqrt(1.0 + ps2m1);
-  double rr = 1.0 / (Ps * (Ps + 1.0));
-  double iPs = rr * (Ps + 1.0), iPs1 = rr * Ps;
-  double tnum = (c.tA - pt2 * r.ibeta0 - z.Pt * ps2m1 * iPs1) * iPs1 * iPs;   // T' of the drift
-  double bx, by, ox, oy, os;
-  mult_field(e, z.X, z.Y, bx, by);
-  omega_straight(z.Px, z.Py, iPs, bx, by, c, ox, oy, os);
-  acc.edge(0, hds * ox, hds * oy, hds * os);
-  for (int i = 1; i <= N; ++i) {
-    z.X = fma(hds * iPs, z.Px, z.X);
-    z.Y = fma(hds * iPs, z.Py, z.Y);
-    z.T = fma(hds, tnum, z.T);
-    mult_field(e, z.X, z.Y, bx, by);
-    z.Px = fma(-ds, by, z.Px);
-    z.Py = fma(ds, bx, z.Py);
-    pt2 = fma(z.Px, z.Px, z.Py * z.Py);
-    ps2m1 = c.e0 - pt2;
-    if (!(1.0 + ps2m1 > 0.0)) return false;
-    Ps = sqrt(1.0 + ps2m1);
-    rr = 1.0 / (Ps * (Ps + 1.0));
-    iPs = rr * (Ps + 1.0); iPs1 = rr * Ps;
-    tnum = (c.tA - pt2 * r.ibeta0 - z.Pt * ps2m1 * iPs1) * iPs1 * iPs;
-    z.X = fma(hds * iPs, z.Px, z.X);
-    z.Y = fma(hds * iPs, z.Py, z.Y);
-    z.T = fma(hds, tnum, z.T);
-    mult_field(e, z.X, z.Y, bx, by);
-    omega_straight(z.Px, z.Py, iPs, bx, by, c, ox, oy, os);
-    double w = (i == N) ? hds : ds;
-    acc.edge(i, w * ox, w * oy, w * os);
+  if (e.pure_quad) {
+    MultDK<true> s(z, e, c, r);
+    run_thick<DEPTH>(s, e.N, e.ds, z.Sx, z.Sy, z.Ss);
+    return !s.bad;
   }
-  acc.finish(z.Sx, z.Sy, z.Ss);
-  return true;
+  MultDK<false> s(z, e, c, r);
+  run_thick<DEPTH>(s, e.N, e.ds, z.Sx, z.Sy, z.Ss);
+  return !s.bad;
 }
 
 // a6: quadrupole matrix-kick (24)(25)(27).  kappa^2 = |k1|/P (23); with u = (kappa ds/2)^2 the four
 // functions cos, sin(x)/x, cosh, sinh(x)/x are power series in u (no sqrt of kappa is needed).
 struct QuadLin {
-  double C, S, Ch, Sh;        // cos x, s*sin(x)/x ... see build()
+  double C, S, Ch, Sh;        // cos x, (s/P) sin(x)/x, cosh x, (s/P) sinh(x)/x
   double kS, kSh;             // |k1| s sin(x)/x,  |k1| s sinh(x)/x
   double tpp_f, txx_f, txp_f; // (24e) coefficients of Px^2, X^2, X Px in the focusing plane
   double tpp_d, txx_d, txp_d; // ... of Py^2, Y^2, Y Py in the defocusing plane
@@ -473,63 +608,80 @@ __device__ __forceinline__ void quadlin_apply(const QuadLin& q, double& uf, doub
   pd = fma(pd, q.Ch, q.kSh * ud);
   ud = nu;
 }
-template <int DEPTH>
-__device__ __forceinline__ bool quad_mk(State& z, const DevElem& e, const PCon& c) {
-  const double k1 = e.kn[0];
-  const bool foc = k1 > 0.0;
-  const int N = e.N;
-  const double ds = e.ds, hds = 0.5 * e.ds;
+template <bool FOC> struct QuadMK {
+  State& z;
+  const PCon& c;
   QuadLin ql;
-  quadlin_build(ql, fabs(k1), hds, c);
-  const double tfac = c.iP * c.ibpt;
-  const double P2 = 1.0 + c.e0;
-  const double hiP3 = 0.5 * c.iP * c.iP * c.iP;
-  SpinAcc<DEPTH> acc;
-  acc.reset();
-  double ox, oy, os;
-  {
-    double ps2 = P2 - fma(z.Px, z.Px, z.Py * z.Py);
-    if (!(ps2 > 0.0)) return false;
-    double iPs = rsqrt(ps2);
-    omega_straight(z.Px, z.Py, iPs, k1 * z.Y, k1 * z.X, c, ox, oy, os);
-    acc.edge(0, hds * ox, hds * oy, hds * os);
+  double k1, ds, tfac, P2, hiP3, a1k;
+  bool bad;
+  __device__ __forceinline__ QuadMK(State& z_, const DevElem& e, const PCon& c_) : z(z_), c(c_) {
+    k1 = e.kn[0];
+    ds = e.ds;
+    quadlin_build(ql, fabs(k1), 0.5 * e.ds, c);
+    tfac = c.iP * c.ibpt;
+    P2 = 1.0 + c.e0;
+    hiP3 = 0.5 * c.iP * c.iP * c.iP;
+    a1k = c.a1 * k1;
+    bad = false;
   }
-  for (int i = 1; i <= N; ++i) {
-    if (foc) quadlin_apply(ql, z.X, z.Px, z.Y, z.Py, z.T, tfac);
+  __device__ __forceinline__ void lin() {
+    if (FOC) quadlin_apply(ql, z.X, z.Px, z.Y, z.Py, z.T, tfac);
     else     quadlin_apply(ql, z.Y, z.Py, z.X, z.Px, z.T, tfac);
+  }
+  __device__ __forceinline__ void advance() {
+    lin();
     {   // (25): X += ds Px (1/Ps - 1/P), 1/Ps - 1/P = pt2/(P Ps (P+Ps))
-      double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
-      double ps2 = P2 - pt2;
-      if (!(ps2 > 0.0)) return false;
-      double Ps = sqrt(ps2);
-      double t = 1.0 / (Ps * (c.P + Ps));           // 1/(Ps (P+Ps))
-      double d = pt2 * c.iP * t;
+      const double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
+      const double ps2 = P2 - pt2;
+      bad |= !(ps2 > 0.0);
+      const double iPs = rsqrt_nr(ps2);
+      const double Ps = ps2 * iPs;
+      const double t = iPs * rcp_nr(c.P + Ps);         // 1/(Ps (P+Ps))
+      const double d = pt2 * c.iP * t;
       z.X = fma(ds * d, z.Px, z.X);
       z.Y = fma(ds * d, z.Py, z.Y);
       // T' = -(1/beta0+Pt)[1/Ps - 1/P - pt2/(2P^3)] + tq,  bracket = pt2^2 (2P+Ps)/(2 P^3 Ps (P+Ps)^2)
-      double br = pt2 * pt2 * fma(2.0, c.P, Ps) * hiP3 * t * (t * Ps);
+      const double br = pt2 * pt2 * fma(2.0, c.P, Ps) * hiP3 * t * (t * Ps);
       z.T = fma(ds, fma(-c.ibpt, br, c.tq), z.T);
     }
-    if (foc) quadlin_apply(ql, z.X, z.Px, z.Y, z.Py, z.T, tfac);
-    else     quadlin_apply(ql, z.Y, z.Py, z.X, z.Px, z.T, tfac);
-    double ps2 = P2 - fma(z.Px, z.Px, z.Py * z.Py);
-    if (!(ps2 > 0.0)) return false;
-    double iPs = rsqrt(ps2);
-    omega_straight(z.Px, z.Py, iPs, k1 * z.Y, k1 * z.X, c, ox, oy, os);
-    double w = (i == N) ? hds : ds;
-    acc.edge(i, w * ox, w * oy, w * os);
+    lin();
   }
-  acc.finish(z.Sx, z.Sy, z.Ss);
-  return true;
+  __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) {
+    const double ps2 = P2 - fma(z.Px, z.Px, z.Py * z.Py);
+    bad |= !(ps2 > 0.0);
+    const double iPs = rsqrt_nr(ps2);
+    const double pb = c.a2p * k1 * (z.Px * z.Y + z.Py * z.X);
+    const double wi = -w * iPs;
+    wx = wi * fma(a1k, z.Y, -pb * z.Px);
+    wy = wi * fma(a1k, z.X, -pb * z.Py);
+    ws = w * pb;
+  }
+};
+template <int DEPTH>
+__device__ __forceinline__ bool quad_mk(State& z, const DevElem& e, const PCon& c) {
+  if (e.kn[0] > 0.0) {
+    QuadMK<true> s(z, e, c);
+    run_thick<DEPTH>(s, e.N, e.ds, z.Sx, z.Sy, z.Ss);
+    return !s.bad;
+  }
+  QuadMK<false> s(z, e, c);
+  run_thick<DEPTH>(s, e.N, e.ds, z.Sx, z.Sy, z.Ss);
+  return !s.bad;
 }
 
 // ---------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------
+// 64-thread blocks, <= 128 registers: the register file is split per SM sub-partition (16 384 each), so
+// 128 registers allow 4 warps per sub-partition = 8 blocks per SM, and the 1024 blocks of a 65 536-
+// particle bunch are resident in ONE wave (148 x 8 = 1184 slots).  With 144+ registers only 3 warps
+// fit per sub-partition (888 slots) and the last 136 blocks run alone in a second wave (measured:
+// 85 ms vs 53 ms per 20 turns, profiles/r01_notes.md).
 constexpr int TRACK_BLOCK = 64;
+constexpr int TRACK_MIN_BLOCKS = 8;
 
 template <int SPLIT, int DEPTH>
-__global__ void __launch_bounds__(TRACK_BLOCK) track_kernel(const TrackArgs a) {
+__global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_kernel(const TrackArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   DevElem* tab = reinterpret_cast<DevElem*>(smem_raw);
   const uint16_t* seq = a.seq;
@@ -571,14 +723,14 @@ __global__ void __launch_bounds__(TRACK_BLOCK) track_kernel(const TrackArgs a) {
           break;
         case K_MULT: alive = mult_dk<DEPTH>(z, e, pc, ref); break;
         case K_THIN: {   // A10: half kick, spin, half kick
-          double bx, by, ox, oy, os;
+          double bx, by, wx, wy, ws;
           mult_field(e, z.X, z.Y, bx, by);
           z.Px = fma(-0.5, by, z.Px);
           z.Py = fma(0.5, bx, z.Py);
           double ps2 = 1.0 + pc.e0 - fma(z.Px, z.Px, z.Py * z.Py);
           if (!(ps2 > 0.0)) { alive = false; break; }
-          omega_straight(z.Px, z.Py, rsqrt(ps2), bx, by, pc, ox, oy, os);
-          Quat q = quat_from_rotvec(ox, oy, os);
+          omega_straight(1.0, z.Px, z.Py, rsqrt_nr(ps2), bx, by, pc, wx, wy, ws);
+          Quat q = quat_from_rotvec(wx, wy, ws);
           quat_rotate(q, z.Sx, z.Sy, z.Ss);
           z.Px = fma(-0.5, by, z.Px);
           z.Py = fma(0.5, bx, z.Py);
