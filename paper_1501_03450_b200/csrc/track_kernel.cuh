@@ -76,23 +76,18 @@ struct Quat { double w, x, y, s; };
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ double rcp_nr(double x) {
   double y;
-  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));   // MUFU.RCP64H: relative error < 2^-20
   double e = fma(-x, y, 1.0);
-  e = fma(e, e, e);                 // e + e^2: one cubic step  y (1 + e + e^2)
-  y = fma(y, e, y);                 // relative error ~2^-60
-  e = fma(-x, y, 1.0);
-  return fma(y, e, y);              // polish to ~1 ulp
+  e = fma(e, e, e);                 // e + e^2: cubic step y (1 + e + e^2), residual e^3 < 2^-60
+  return fma(y, e, y);              // ~1 ulp (gst_selftest_math measures it)
 }
 __device__ __forceinline__ double rsqrt_nr(double x) {
   double y;
-  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x)); // MUFU.RSQ64H: relative error < 2^-20
   double t = x * y;
   double e = fma(-t, y, 1.0);       // 1 - x y^2
   double c = fma(0.375, e, 0.5);
-  y = fma(y * e, c, y);             // cubic step, relative error ~2^-58
-  t = x * y;
-  e = fma(-t, y, 1.0);
-  return fma(0.5 * y, e, y);        // polish to ~1 ulp
+  return fma(y * e, c, y);          // cubic step y (1 + e/2 + 3e^2/8), residual (5/16) e^3 < 2^-58
 }
 
 // reference-particle and per-particle constants that change only when Pt or E0 changes
@@ -138,44 +133,58 @@ __device__ __forceinline__ void pcon_set(PCon& c, double Pt, const Ref& r, doubl
 // q = (cos(th/2), sin(th/2) w/th) for rotation vector w: both factors are even in th, so they are
 // power series in v = th^2 -- no sqrt, no division, no sincos ("low-order polynomials", here
 // taken to full double precision).  Three tiers by angle; the first is the straight-line path.
+// The coefficients sit in constant memory so that each DFMA takes its coefficient as a c[bank][offset]
+// operand (a double literal would cost two extra UMOV/MOV instructions per use on sm_100).
+//   QPOLY[2k]   = (-1/4)^k/(2k)!        (cos x,        x^2 = v/4)
+//   QPOLY[2k+1] = (1/2)(-1/4)^k/(2k+1)!  (sin(x)/th)
+__constant__ double QPOLY[14] = {
+    1.0, 0.5,
+    -1.0 / 8.0, -0.5 / 24.0,
+    1.0 / (16.0 * 24.0), 0.5 / (16.0 * 120.0),
+    -1.0 / (64.0 * 720.0), -0.5 / (64.0 * 5040.0),
+    1.0 / (256.0 * 40320.0), 0.5 / (256.0 * 362880.0),
+    -1.0 / (1024.0 * 3628800.0), -0.5 / (1024.0 * 39916800.0),
+    1.0 / (4096.0 * 479001600.0), 0.5 / (4096.0 * 6227020800.0)};
+
+// tiers 2 and 3 (large angle per edge), kept out of line: they are rare and would otherwise be
+// replicated at every call site (instruction-cache footprint)
+__device__ __noinline__ double2 quat_cs_slow(double v) {
+  double c, s;
+  if (v <= 2.0) {
+    // tier 2: u = v/4 <= 0.5, k = 0..9, remainder < 4e-20
+    double u = 0.25 * v;
+    c = -1.0 / 6402373705728000.0;  s = -1.0 / 121645100408832000.0;
+    c = fma(c, u, 1.0 / 20922789888000.0);  s = fma(s, u, 1.0 / 355687428096000.0);
+    c = fma(c, u, -1.0 / 87178291200.0);    s = fma(s, u, -1.0 / 1307674368000.0);
+    c = fma(c, u, 1.0 / 479001600.0);       s = fma(s, u, 1.0 / 6227020800.0);
+    c = fma(c, u, -1.0 / 3628800.0);        s = fma(s, u, -1.0 / 39916800.0);
+    c = fma(c, u, 1.0 / 40320.0);           s = fma(s, u, 1.0 / 362880.0);
+    c = fma(c, u, -1.0 / 720.0);            s = fma(s, u, -1.0 / 5040.0);
+    c = fma(c, u, 1.0 / 24.0);              s = fma(s, u, 1.0 / 120.0);
+    c = fma(c, u, -0.5);                    s = fma(s, u, -1.0 / 6.0);
+    c = fma(c, u, 1.0);                     s = fma(s, u, 1.0);
+    s *= 0.5;
+  } else {
+    double th = sqrt(v), sn, cs;
+    sincos(0.5 * th, &sn, &cs);
+    c = cs; s = sn / th;
+  }
+  return make_double2(c, s);
+}
+
 __device__ __forceinline__ Quat quat_from_rotvec(double wx, double wy, double ws) {
   const double v = fma(wx, wx, fma(wy, wy, ws * ws));   // th^2;  x = th/2, x^2 = v/4
-  // tier 1: v <= 0.5 (th <= 0.707): cos x = sum_k (-v/4)^k/(2k)!, sin(x)/th = (1/2) sum_k (-v/4)^k/(2k+1)!,
-  // k = 0..6, remainder (v/4)^7/14! < 6e-18
-  double c = 1.0 / (4096.0 * 479001600.0);              // + (v/4)^6/12!
-  double s = 0.5 / (4096.0 * 6227020800.0);             // + (1/2)(v/4)^6/13!
-  c = fma(c, v, -1.0 / (1024.0 * 3628800.0));
-  s = fma(s, v, -0.5 / (1024.0 * 39916800.0));
-  c = fma(c, v, 1.0 / (256.0 * 40320.0));
-  s = fma(s, v, 0.5 / (256.0 * 362880.0));
-  c = fma(c, v, -1.0 / (64.0 * 720.0));
-  s = fma(s, v, -0.5 / (64.0 * 5040.0));
-  c = fma(c, v, 1.0 / (16.0 * 24.0));
-  s = fma(s, v, 0.5 / (16.0 * 120.0));
-  c = fma(c, v, -1.0 / 8.0);
-  s = fma(s, v, -0.5 / 24.0);
-  c = fma(c, v, 1.0);
-  s = fma(s, v, 0.5);
+  // tier 1: v <= 0.5 (th <= 0.707), k = 0..6, remainder (v/4)^7/14! < 6e-18
+  double c = QPOLY[12], s = QPOLY[13];
+  c = fma(c, v, QPOLY[10]); s = fma(s, v, QPOLY[11]);
+  c = fma(c, v, QPOLY[8]);  s = fma(s, v, QPOLY[9]);
+  c = fma(c, v, QPOLY[6]);  s = fma(s, v, QPOLY[7]);
+  c = fma(c, v, QPOLY[4]);  s = fma(s, v, QPOLY[5]);
+  c = fma(c, v, QPOLY[2]);  s = fma(s, v, QPOLY[3]);
+  c = fma(c, v, 1.0);       s = fma(s, v, 0.5);
   if (__builtin_expect(v > 0.5, 0)) {
-    if (v <= 2.0) {
-      // tier 2: u = v/4 <= 0.5, k = 0..9, remainder < 4e-20
-      double u = 0.25 * v;
-      c = -1.0 / 6402373705728000.0;  s = -1.0 / 121645100408832000.0;
-      c = fma(c, u, 1.0 / 20922789888000.0);  s = fma(s, u, 1.0 / 355687428096000.0);
-      c = fma(c, u, -1.0 / 87178291200.0);    s = fma(s, u, -1.0 / 1307674368000.0);
-      c = fma(c, u, 1.0 / 479001600.0);       s = fma(s, u, 1.0 / 6227020800.0);
-      c = fma(c, u, -1.0 / 3628800.0);        s = fma(s, u, -1.0 / 39916800.0);
-      c = fma(c, u, 1.0 / 40320.0);           s = fma(s, u, 1.0 / 362880.0);
-      c = fma(c, u, -1.0 / 720.0);            s = fma(s, u, -1.0 / 5040.0);
-      c = fma(c, u, 1.0 / 24.0);              s = fma(s, u, 1.0 / 120.0);
-      c = fma(c, u, -0.5);                    s = fma(s, u, -1.0 / 6.0);
-      c = fma(c, u, 1.0);                     s = fma(s, u, 1.0);
-      s *= 0.5;
-    } else {
-      double th = sqrt(v), sn, cs;
-      sincos(0.5 * th, &sn, &cs);
-      c = cs; s = sn / th;
-    }
+    const double2 cs = quat_cs_slow(v);
+    c = cs.x; s = cs.y;
   }
   return Quat{c, s * wx, s * wy, s * ws};
 }
@@ -366,6 +375,8 @@ struct BendExact {
   }
 };
 
+__constant__ double APOLY[6] = {1.0 / 6.0, 3.0 / 40.0, 15.0 / 336.0, 105.0 / 3456.0, 945.0 / 42240.0, 10395.0 / 599040.0};
+
 template <int DEPTH>
 __device__ __forceinline__ bool sbend_exact(State& z, const DevElem& e, const PCon& c, const Ref& r) {
   BendExact s(z, e, c);
@@ -376,12 +387,12 @@ __device__ __forceinline__ bool sbend_exact(State& z, const DevElem& e, const PC
   const double v = x * x;
   double dasin;
   if (v < 2.5e-3) {     // asin(x)/x = 1 + v/6 + 3v^2/40 + 15v^3/336 + 105v^4/3456 + 945v^5/42240 + 10395v^6/599040
-    double p = 10395.0 / 599040.0;
-    p = fma(p, v, 945.0 / 42240.0);
-    p = fma(p, v, 105.0 / 3456.0);
-    p = fma(p, v, 15.0 / 336.0);
-    p = fma(p, v, 3.0 / 40.0);
-    p = fma(p, v, 1.0 / 6.0);
+    double p = APOLY[5];
+    p = fma(p, v, APOLY[4]);
+    p = fma(p, v, APOLY[3]);
+    p = fma(p, v, APOLY[2]);
+    p = fma(p, v, APOLY[1]);
+    p = fma(p, v, APOLY[0]);
     dasin = fma(p * v, x, x);
   } else {
     dasin = asin(x);
@@ -482,17 +493,16 @@ template <bool PURE> struct MultDK {
   State& z;
   const DevElem& e;
   const PCon& c;
-  double iPs, tnum, hds, k1, dsk, a1k, ibeta0;
+  double iPs, tnum, hds, k1, dsk, a1k, ibeta0, P2;
   bool bad;
+  // T' = 1/beta0 - (1/beta0+Pt)/Ps is formed directly here: its rounding error is 2^-53 * (ds/2) per half
+  // drift in ABSOLUTE terms (a few 1e-18 m), far below 1e-12 of any bunch length;
+  // the cancellation-free form (one more MUFU + 14 FP64 instructions per slice) is kept for whole drifts.
   __device__ __forceinline__ void momenta() {
-    const double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
-    const double ps2m1 = c.e0 - pt2;
-    const double ps2 = 1.0 + ps2m1;
+    const double ps2 = P2 - fma(z.Px, z.Px, z.Py * z.Py);
     bad |= !(ps2 > 0.0);
     iPs = rsqrt_nr(ps2);
-    const double Ps = ps2 * iPs;
-    const double iPs1 = rcp_nr(Ps + 1.0);
-    tnum = (fma(-pt2, ibeta0, c.tA) - z.Pt * ps2m1 * iPs1) * iPs1 * iPs;   // T' of the drift
+    tnum = fma(-c.ibpt, iPs, ibeta0);
   }
   __device__ __forceinline__ MultDK(State& z_, const DevElem& e_, const PCon& c_, const Ref& r) : z(z_), e(e_), c(c_) {
     hds = 0.5 * e.ds;
@@ -500,6 +510,7 @@ template <bool PURE> struct MultDK {
     dsk = e.ds * k1;
     a1k = c.a1 * k1;
     ibeta0 = r.ibeta0;
+    P2 = 1.0 + c.e0;
     bad = false;
     momenta();
   }
