@@ -128,6 +128,11 @@ gst_status gst_track_host(const gst_lattice* lat, double* const host_state[9], s
  * FP64 (CUDA-core) peak the roofline is reported against.  HOST out: TFLOP/s (2 flop per DFMA).   */
 gst_status gst_fp64_peak(double* out_tflops, double* out_ms);
 
+/* Accuracy self-test of the kernels' branch-free reciprocal and reciprocal square root (MUFU seed +
+ * one cubic Newton step) over 2^24 arguments in [0.25, 4): HOST out = {max |x*rcp(x) - 1|,
+ * max |sqrt(x)*rsqrt(x) - 1|} in units of 2^-53.                                                   */
+gst_status gst_selftest_math(double out[2]);
+
 /* Thread-local message for the last error on this thread; never NULL. */
 const char* gst_last_error(void);
 

@@ -150,6 +150,21 @@ gst_status get_table(const gst_lattice* lat, int n_slices, const gst::DevElem** 
   return GST_OK;
 }
 
+// max relative error (in units of 2^-53) of the branch-free reciprocal / reciprocal square root
+__global__ void math_selftest_kernel(unsigned long long* out, int n) {
+  double worst_rcp = 0.0, worst_rsq = 0.0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    double x = exp2(-2.0 + 4.0 * ((double)i + 0.37) / (double)n);     // [0.25, 4)
+    double r = gst::rcp_nr(x), q = gst::rsqrt_nr(x);
+    double er = fabs(fma(r, x, -1.0));                                 // |r x - 1|, exact residual
+    double eq = fabs(fma(q * q, x, -1.0)) * 0.5;                       // ~ |q sqrt(x) - 1|
+    worst_rcp = fmax(worst_rcp, er);
+    worst_rsq = fmax(worst_rsq, eq);
+  }
+  atomicMax(out, (unsigned long long)__double_as_longlong(worst_rcp));
+  atomicMax(out + 1, (unsigned long long)__double_as_longlong(worst_rsq));
+}
+
 template <int SPLIT, int DEPTH>
 cudaError_t launch_track(const gst::TrackArgs& a, size_t smem, cudaStream_t st) {
   auto kern = gst::track_kernel<SPLIT, DEPTH>;
@@ -439,6 +454,24 @@ gst_status gst_track_host(const gst_lattice* lat, double* const host_state[9], s
   cudaStreamDestroy(st);
   cudaFree(d);
   return s;
+}
+
+gst_status gst_selftest_math(double out[2]) {
+  if (!out) return fail(GST_EINVAL, "null argument");
+  unsigned long long* d = nullptr;
+  CUDA_TRY(cudaMalloc(&d, 16));
+  CUDA_TRY(cudaMemset(d, 0, 16));
+  math_selftest_kernel<<<296, 256>>>(d, 1 << 24);
+  unsigned long long h[2];
+  cudaError_t ce = cudaMemcpy(h, d, 16, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (ce != cudaSuccess) return fail(GST_ECUDA, "selftest: %s", cudaGetErrorString(ce));
+  for (int k = 0; k < 2; ++k) {
+    double v;
+    std::memcpy(&v, &h[k], 8);
+    out[k] = v / 1.1102230246251565e-16;      // in units of 2^-53
+  }
+  return GST_OK;
 }
 
 gst_status gst_fp64_peak(double* out_tflops, double* out_ms) {

@@ -35,18 +35,28 @@ WANT = {
 
 
 def read_raw(path):
-    rows = list(csv.reader(open(path)))
-    hdr = next(i for i, r in enumerate(rows) if r and r[0] == "ID")
-    names, units, vals = rows[hdr], rows[hdr + 1], rows[hdr + 2]
+    """Accepts both ncu CSV layouts: `--page raw --csv` (wide: one column per metric) and
+    `--csv --metrics ...` (long: one row per metric).  Lines before the header (==PROF== ...) are skipped."""
+    rows = [r for r in csv.reader(open(path)) if r]
+    hdr = next(i for i, r in enumerate(rows) if r[0] == "ID")
+    names = rows[hdr]
     out = {}
-    for n, u, v in zip(names, units, vals):
-        out[n] = (v, u)
+    if "Metric Name" in names:
+        kn, ku, kv = names.index("Metric Name"), names.index("Metric Unit"), names.index("Metric Value")
+        first = rows[hdr + 1][0]
+        for r in rows[hdr + 1:]:
+            if r[0] == first and len(r) > kv:
+                out[r[kn]] = (r[kv], r[ku])
+    else:
+        units, vals = rows[hdr + 1], rows[hdr + 2]
+        for n, u, v in zip(names, units, vals):
+            out[n] = (v, u)
     return out
 
 
 def to_float(v, u):
     x = float(v.replace(",", ""))
-    scale = {"Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "byte": 1, "usecond": 1e3, "msecond": 1e6, "nsecond": 1,
+    scale = {"Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "byte": 1, "inst": 1, "usecond": 1e3, "msecond": 1e6, "nsecond": 1,
              "second": 1e9, "us": 1e3, "ms": 1e6, "ns": 1, "s": 1e9}
     return x * scale.get(u, 1)
 

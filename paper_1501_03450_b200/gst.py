@@ -38,7 +38,7 @@ _dp = C.POINTER(C.c_double)
 
 EXPORTS = ["gst_lattice_create", "gst_lattice_destroy", "gst_lattice_steps_per_turn", "gst_bunch_init",
            "gst_bunch_destroy", "gst_track", "gst_polarization", "gst_emittance", "gst_bunch_lost",
-           "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host", "gst_fp64_peak", "gst_last_error"]
+           "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host", "gst_fp64_peak", "gst_selftest_math", "gst_last_error"]
 
 
 def lib():
@@ -68,6 +68,8 @@ def lib():
         L.gst_track_host.argtypes = [vp, C.POINTER(_dp), C.c_size_t, C.c_int64, C.c_int, C.c_int, C.c_int, _dp,
                                      C.POINTER(C.c_int64)]
         L.gst_fp64_peak.argtypes = [_dp, _dp]
+        L.gst_selftest_math.argtypes = [_dp]
+        L.gst_selftest_math.restype = C.c_int
         for name in ("gst_lattice_create", "gst_bunch_init", "gst_track", "gst_polarization", "gst_emittance",
                      "gst_bunch_lost", "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host",
                      "gst_fp64_peak"):
@@ -214,3 +216,10 @@ def fp64_peak():
     ms = C.c_double(0)
     _check(lib().gst_fp64_peak(C.byref(t), C.byref(ms)))
     return t.value, ms.value
+
+
+def selftest_math():
+    """gst_selftest_math: max residuals of the kernels' rcp / rsqrt in units of 2^-53."""
+    out = (C.c_double * 2)()
+    _check(lib().gst_selftest_math(out))
+    return out[0], out[1]

@@ -287,3 +287,8 @@ def test_config3_full_size_sampled_particles(gst, O):
     # properties that hold at any size: unit spins, snakes keep the bunch polarized near the vertical
     assert np.max(np.abs(np.linalg.norm(got[6:9], axis=0) - 1)) < 1e-11
     assert abs(pol[3] - np.linalg.norm(got[6:9].mean(axis=1))) < 1e-12
+
+
+def test_branch_free_rcp_and_rsqrt_are_accurate_to_a_few_ulp(gst):
+    rcp, rsq = gst.selftest_math()
+    assert 0 < rcp < 4.0 and 0 < rsq < 4.0, (rcp, rsq)
