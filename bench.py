@@ -113,7 +113,7 @@ def cpu_baseline(cfg, budget_s=15.0):
     t0 = time.perf_counter()
     O.track(lat, beam, st, 1, cfg["split"], cfg["n_slices"], cfg["depth"], prec=O.PREC_DOUBLE, threads=cores)
     t1 = time.perf_counter() - t0
-    turns = int(max(2, min(200, budget_s / max(t1, 1e-3))))
+    turns = int(max(2, min(20000, budget_s / max(t1, 1e-3))))
     t0 = time.perf_counter()
     O.track(lat, beam, st, turns, cfg["split"], cfg["n_slices"], cfg["depth"], prec=O.PREC_DOUBLE, threads=cores)
     dt = time.perf_counter() - t0
