@@ -103,6 +103,13 @@ void gst_bunch_destroy(gst_bunch* b);
 gst_status gst_track(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, gst_split split, int n_slices,
                      int romberg_depth, void* cuda_stream);
 
+/* Which tracking kernel gst_track launches (process-wide; results are bit-identical):
+ *   GST_KERNEL_FUSED  one thread per particle, orbit and spin work software-pipelined -- default
+ *   GST_KERNEL_PAIR   experimental: an orbit thread and a spin thread per particle, coupled through a
+ *                     shared-memory ring (csrc/track_pair_kernel.cuh); slower on B200 as measured      */
+typedef enum { GST_KERNEL_FUSED = 0, GST_KERNEL_PAIR = 1 } gst_kernel_variant;
+gst_status gst_set_kernel_variant(gst_kernel_variant v);
+
 /* Bunch polarization (a13; reading A18): out = {Px, Py, Ps, |P|} over particles not lost;
  * out_lost (may be NULL) = number lost.  Enqueues the reduction on the stream and SYNCHRONISES it.
  * `out` and `out_lost` are HOST pointers.                                                           */

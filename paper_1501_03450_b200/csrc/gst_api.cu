@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <atomic>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -16,10 +17,12 @@
 
 #include "reduce_kernel.cuh"
 #include "track_kernel.cuh"
+#include "track_pair_kernel.cuh"
 
 namespace {
 
 thread_local std::string g_err = "";
+std::atomic<int> g_variant{GST_KERNEL_FUSED};
 
 gst_status fail(gst_status s, const char* fmt, ...) {
   char buf[512];
@@ -165,27 +168,61 @@ __global__ void math_selftest_kernel(unsigned long long* out, int n) {
   atomicMax(out + 1, (unsigned long long)__double_as_longlong(worst_rsq));
 }
 
+// shared memory of one block: [ring + lost flags (pair kernel only)] table [sequence when it fits]
+struct SmemPlan { size_t bytes; int use_smem_seq; };
+SmemPlan plan_smem(size_t tab_bytes, size_t seq_bytes, size_t fixed, size_t budget) {
+  SmemPlan p;
+  p.use_smem_seq = (fixed + tab_bytes + seq_bytes <= budget) ? 1 : 0;
+  p.bytes = fixed + tab_bytes + (p.use_smem_seq ? seq_bytes : 0);
+  return p;
+}
+
 template <int SPLIT, int DEPTH>
-cudaError_t launch_track(const gst::TrackArgs& a, size_t smem, cudaStream_t st) {
+cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, bool pair, cudaStream_t st) {
+  if (pair) {
+    // T1p: two threads per particle.  Shared memory per block is budgeted so that MIN_BLOCKS blocks stay
+    // resident per SM (227 kB usable, 1 kB reserved per block).
+    using Cfg = gst::PairCfg<DEPTH>;
+    auto kern = gst::track_pair_kernel<SPLIT, DEPTH>;
+    const size_t fixed = (size_t)Cfg::PAIRS * (gst::PAIR_RING_BYTES + 32);
+    const size_t budget = (size_t)(227 * 1024) / Cfg::MIN_BLOCKS - 1024;
+    SmemPlan p = plan_smem(tab_bytes, seq_bytes, fixed, budget);
+
+    a.use_smem_seq = p.use_smem_seq;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
+    if (e != cudaSuccess) return e;
+    // ask for just enough shared memory for MIN_BLOCKS blocks; the rest of the 228 kB stays L1
+    int carve = (int)(((p.bytes + 1024) * Cfg::MIN_BLOCKS * 100 + 228 * 1024 - 1) / (228 * 1024));
+    if (carve > 100) carve = 100;
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, carve);
+    if (e != cudaSuccess) return e;
+    const long long per_block = 32LL * Cfg::PAIRS;
+    unsigned blocks = (unsigned)((a.n + per_block - 1) / per_block);
+    kern<<<blocks, Cfg::THREADS, p.bytes, st>>>(a);
+    return cudaGetLastError();
+  }
+  // T1: one thread per particle; shared memory kept small so that 8 blocks of 64 threads stay resident
   auto kern = gst::track_kernel<SPLIT, DEPTH>;
-  if (smem > 48 * 1024) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  SmemPlan p = plan_smem(tab_bytes, seq_bytes, 0, 24 * 1024);
+  a.use_smem_seq = p.use_smem_seq;
+  if (p.bytes > 48 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
     if (e != cudaSuccess) return e;
   }
   unsigned blocks = (unsigned)((a.n + gst::TRACK_BLOCK - 1) / gst::TRACK_BLOCK);
-  kern<<<blocks, gst::TRACK_BLOCK, smem, st>>>(a);
+  kern<<<blocks, gst::TRACK_BLOCK, p.bytes, st>>>(a);
   return cudaGetLastError();
 }
 
 template <int SPLIT>
-cudaError_t launch_track_depth(int depth, const gst::TrackArgs& a, size_t smem, cudaStream_t st) {
+cudaError_t launch_track_depth(int depth, const gst::TrackArgs& a, size_t tb, size_t sb, bool pair, cudaStream_t st) {
   switch (depth) {
-    case 1: return launch_track<SPLIT, 1>(a, smem, st);
-    case 2: return launch_track<SPLIT, 2>(a, smem, st);
-    case 3: return launch_track<SPLIT, 3>(a, smem, st);
-    case 4: return launch_track<SPLIT, 4>(a, smem, st);
-    case 5: return launch_track<SPLIT, 5>(a, smem, st);
-    default: return launch_track<SPLIT, 6>(a, smem, st);
+    case 1: return launch_track<SPLIT, 1>(a, tb, sb, pair, st);
+    case 2: return launch_track<SPLIT, 2>(a, tb, sb, pair, st);
+    case 3: return launch_track<SPLIT, 3>(a, tb, sb, pair, st);
+    case 4: return launch_track<SPLIT, 4>(a, tb, sb, pair, st);
+    case 5: return launch_track<SPLIT, 5>(a, tb, sb, pair, st);
+    default: return launch_track<SPLIT, 6>(a, tb, sb, pair, st);
   }
 }
 
@@ -208,6 +245,12 @@ gst_status validate_track(const gst_lattice* lat, int64_t n_turns, int split, in
 extern "C" {
 
 const char* gst_last_error(void) { return g_err.c_str(); }
+
+gst_status gst_set_kernel_variant(gst_kernel_variant v) {
+  if (v != GST_KERNEL_FUSED && v != GST_KERNEL_PAIR) return fail(GST_EINVAL, "unknown kernel variant %d", (int)v);
+  g_variant.store((int)v);
+  return GST_OK;
+}
 
 gst_status gst_lattice_create(const gst_element* elems, size_t n, const gst_beam* beam, gst_lattice** out) {
   if (!elems || !beam || !out || n == 0) return fail(GST_EINVAL, "null argument or empty lattice");
@@ -345,17 +388,15 @@ gst_status gst_track(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, gst_
   a.G = lat->beam.G;
   size_t tab_bytes = lat->uniq.size() * sizeof(gst::DevElem);
   size_t seq_bytes = (lat->seq.size() * sizeof(uint16_t) + 15) & ~size_t(15);
-  // shared memory per block is kept small so that >= 8 blocks of 64 threads stay resident per SM
-  const size_t tab_cap = 48 * 1024, seq_cap = 24 * 1024;
-  if (tab_bytes > tab_cap) return fail(GST_EINVAL, "too many unique elements for the shared-memory table (%zu)", lat->uniq.size());
-  a.use_smem_seq = (tab_bytes + seq_bytes <= seq_cap) ? 1 : 0;
-  size_t smem = tab_bytes + (a.use_smem_seq ? seq_bytes : 0);
+  if (tab_bytes > 24 * 1024) return fail(GST_EINVAL, "too many unique elements for the shared-memory table (%zu)", lat->uniq.size());
+  const bool pair = g_variant.load() == GST_KERNEL_PAIR;
+  a.use_smem_seq = 0;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   cudaError_t ce;
   switch (split) {
-    case GST_SPLIT_DRIFT_KICK: ce = launch_track_depth<gst::SPLIT_DK>(romberg_depth, a, smem, st); break;
-    case GST_SPLIT_BEND_KICK: ce = launch_track_depth<gst::SPLIT_BK>(romberg_depth, a, smem, st); break;
-    default: ce = launch_track_depth<gst::SPLIT_MK>(romberg_depth, a, smem, st); break;
+    case GST_SPLIT_DRIFT_KICK: ce = launch_track_depth<gst::SPLIT_DK>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
+    case GST_SPLIT_BEND_KICK: ce = launch_track_depth<gst::SPLIT_BK>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
+    default: ce = launch_track_depth<gst::SPLIT_MK>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
   }
   if (ce != cudaSuccess) return fail(GST_ECUDA, "track launch: %s", cudaGetErrorString(ce));
   // host-side bookkeeping of the reference energy: the same IEEE additions the kernel performs

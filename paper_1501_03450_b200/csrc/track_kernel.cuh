@@ -293,40 +293,53 @@ __device__ __forceinline__ bool drift(State& z, double L, const PCon& c, const R
 
 // ---------------------------------------------------------------------------------------------
 // thick elements: a "stepper" advances the orbit by one slice and evaluates weight*ds*Omega at the
-// current point; run_thick drives it through the N slices with the spin work software-pipelined.
+// current point; the spin policy's run() drives it through the N slices with the spin work software-pipelined.
 // ---------------------------------------------------------------------------------------------
-template <int DEPTH, class Stepper>
-__device__ __forceinline__ void run_thick(Stepper& s, int N, double ds, double& Sx, double& Sy, double& Ss) {
-  SpinAcc<DEPTH> acc;
-  acc.reset();
-  const double hds = 0.5 * ds;
-  double wx, wy, ws;
-  s.omega(hds, wx, wy, ws);                       // pending edge 0, half weight
-  if (DEPTH == 1) {
-    for (int i = 1; i <= N; ++i) {
-      s.advance();                                // orbit slice i ...
-      acc.template fold_static<1>(wx, wy, ws);    // ... independent of the spin work of edge i-1
-      s.omega(i == N ? hds : ds, wx, wy, ws);
-    }
-    acc.template fold_static<1>(wx, wy, ws);
-  } else {
-    // DEPTH >= 2: N is even (A4).  Edges are taken in pairs (even, odd): the odd edge belongs to
-    // level 0 only, the even edge to levels 0 and 1 and, where 4 | i, 8 | i, ..., to higher ones.
-    for (int i = 0; i < N; i += 2) {
-      s.advance();
-      {
-        Quat q = acc.template fold_static<2>(wx, wy, ws);    // even edge i
-        acc.template fold_dynamic<2>(i, q);
+// The spin side of a thick element is a policy object with one method, run(stepper, N, ds):
+//   FusedSpin<DEPTH>  -- this thread folds every edge into its own level products (one thread per particle)
+//   PushSpin          -- track_pair_kernel.cuh: the edge rotation vectors go to a partner thread through shared memory
+template <int DEPTH> struct FusedSpin {
+  double &Sx, &Sy, &Ss;
+  __device__ __forceinline__ FusedSpin(State& z) : Sx(z.Sx), Sy(z.Sy), Ss(z.Ss) {}
+  template <class Stepper>
+  __device__ __forceinline__ void run(Stepper& s, int N, double ds) {
+    SpinAcc<DEPTH> acc;
+    acc.reset();
+    const double hds = 0.5 * ds;
+    double wx, wy, ws;
+    s.omega(hds, wx, wy, ws);                       // pending edge 0, half weight
+    if (DEPTH == 1) {
+      for (int i = 1; i <= N; ++i) {
+        s.advance();                                // orbit slice i ...
+        acc.template fold_static<1>(wx, wy, ws);    // ... independent of the spin work of edge i-1
+        s.omega(i == N ? hds : ds, wx, wy, ws);
       }
-      s.omega(ds, wx, wy, ws);
-      s.advance();
-      acc.template fold_static<1>(wx, wy, ws);               // odd edge i+1
-      s.omega(i + 2 == N ? hds : ds, wx, wy, ws);
+      acc.template fold_static<1>(wx, wy, ws);
+    } else {
+      // DEPTH >= 2: N is even (A4).  Edges are taken in pairs (even, odd): the odd edge belongs to
+      // level 0 only, the even edge to levels 0 and 1 and, where 4 | i, 8 | i, ..., to higher ones.
+      for (int i = 0; i < N; i += 2) {
+        s.advance();
+        {
+          Quat q = acc.template fold_static<2>(wx, wy, ws);    // even edge i
+          acc.template fold_dynamic<2>(i, q);
+        }
+        s.omega(ds, wx, wy, ws);
+        s.advance();
+        acc.template fold_static<1>(wx, wy, ws);               // odd edge i+1
+        s.omega(i + 2 == N ? hds : ds, wx, wy, ws);
+      }
+      acc.template fold_static<DEPTH>(wx, wy, ws);             // edge N: every level (2^(DEPTH-1) | N)
     }
-    acc.template fold_static<DEPTH>(wx, wy, ws);             // edge N: every level (2^(DEPTH-1) | N)
+    acc.finish(Sx, Sy, Ss);
   }
-  acc.finish(Sx, Sy, Ss);
-}
+  // thin element (A10): one rotation, no Romberg
+  __device__ __forceinline__ void thin(double wx, double wy, double ws) {
+    Quat q = quat_from_rotvec(wx, wy, ws);
+    quat_rotate(q, Sx, Sy, Ss);
+  }
+  __device__ __forceinline__ void snake(const Quat& q) { quat_rotate(q, Sx, Sy, Ss); }
+};
 
 // a4: exact sector bend (10), spin from the slice-edge Omega (6b).
 // With c = cos(h ds), s = sin(h ds), A = sqrt(Pa^2 - Px^2), g = A - eta(1 + hX):
@@ -377,11 +390,11 @@ struct BendExact {
 
 __constant__ double APOLY[6] = {1.0 / 6.0, 3.0 / 40.0, 15.0 / 336.0, 105.0 / 3456.0, 945.0 / 42240.0, 10395.0 / 599040.0};
 
-template <int DEPTH>
-__device__ __forceinline__ bool sbend_exact(State& z, const DevElem& e, const PCon& c, const Ref& r) {
+template <class Spin>
+__device__ __forceinline__ bool sbend_exact(State& z, const DevElem& e, const PCon& c, const Ref& r, Spin& spin) {
   BendExact s(z, e, c);
   const double A0 = s.A, Am1_0 = s.Am1, Px0 = z.Px;
-  run_thick<DEPTH>(s, e.N, e.ds, z.Sx, z.Sy, z.Ss);
+  spin.run(s, e.N, e.ds);
   // asin(Px0/Pa) - asin(PxN/Pa) = asin(x),  x = (Px0 A_N - Px_N A_0)/Pa^2  (no cancellation)
   const double x = fma(Px0, s.Am1 - Am1_0, -(z.Px - Px0) * A0) * rcp_nr(s.Pa2);
   const double v = x * x;
@@ -456,10 +469,10 @@ struct BendTeapot {
     ws = fq * Ps;
   }
 };
-template <int DEPTH>
-__device__ __forceinline__ bool sbend_teapot(State& z, const DevElem& e, const PCon& c) {
+template <class Spin>
+__device__ __forceinline__ bool sbend_teapot(State& z, const DevElem& e, const PCon& c, Spin& spin) {
   BendTeapot s(z, e, c);
-  run_thick<DEPTH>(s, e.N, e.ds, z.Sx, z.Sy, z.Ss);
+  spin.run(s, e.N, e.ds);
   return !s.bad;
 }
 
@@ -548,15 +561,15 @@ template <bool PURE> struct MultDK {
     }
   }
 };
-template <int DEPTH>
-__device__ __forceinline__ bool mult_dk(State& z, const DevElem& e, const PCon& c, const Ref& r) {
+template <class Spin>
+__device__ __forceinline__ bool mult_dk(State& z, const DevElem& e, const PCon& c, const Ref& r, Spin& spin) {
   if (e.pure_quad) {
     MultDK<true> s(z, e, c, r);
-    run_thick<DEPTH>(s, e.N, e.ds, z.Sx, z.Sy, z.Ss);
+    spin.run(s, e.N, e.ds);
     return !s.bad;
   }
   MultDK<false> s(z, e, c, r);
-  run_thick<DEPTH>(s, e.N, e.ds, z.Sx, z.Sy, z.Ss);
+  spin.run(s, e.N, e.ds);
   return !s.bad;
 }
 
@@ -668,16 +681,65 @@ template <bool FOC> struct QuadMK {
     ws = w * pb;
   }
 };
-template <int DEPTH>
-__device__ __forceinline__ bool quad_mk(State& z, const DevElem& e, const PCon& c) {
+template <class Spin>
+__device__ __forceinline__ bool quad_mk(State& z, const DevElem& e, const PCon& c, Spin& spin) {
   if (e.kn[0] > 0.0) {
     QuadMK<true> s(z, e, c);
-    run_thick<DEPTH>(s, e.N, e.ds, z.Sx, z.Sy, z.Ss);
+    spin.run(s, e.N, e.ds);
     return !s.bad;
   }
   QuadMK<false> s(z, e, c);
-  run_thick<DEPTH>(s, e.N, e.ds, z.Sx, z.Sy, z.Ss);
+  spin.run(s, e.N, e.ds);
   return !s.bad;
+}
+
+// ---------------------------------------------------------------------------------------------
+// one element (the switch is uniform across the grid: every particle is in the same element)
+// ---------------------------------------------------------------------------------------------
+template <int SPLIT, class Spin>
+__device__ __forceinline__ bool element_step(State& z, const DevElem& e, PCon& pc, Ref& ref, double G, Spin& spin) {
+  switch (e.type) {
+    case K_DRIFT: return drift(z, e.L, pc, ref);
+    case K_SBEND:
+      if (SPLIT == SPLIT_DK) return sbend_teapot(z, e, pc, spin);
+      return sbend_exact(z, e, pc, ref, spin);
+    case K_QUAD:
+      if (SPLIT == SPLIT_MK) return quad_mk(z, e, pc, spin);
+      return mult_dk(z, e, pc, ref, spin);
+    case K_MULT: return mult_dk(z, e, pc, ref, spin);
+    case K_THIN: {   // A10: half kick, spin, half kick
+      double bx, by, wx, wy, ws;
+      mult_field(e, z.X, z.Y, bx, by);
+      z.Px = fma(-0.5, by, z.Px);
+      z.Py = fma(0.5, bx, z.Py);
+      const double ps2 = 1.0 + pc.e0 - fma(z.Px, z.Px, z.Py * z.Py);
+      const bool ok = ps2 > 0.0;
+      omega_straight(1.0, z.Px, z.Py, rsqrt_nr(ok ? ps2 : 1.0), bx, by, pc, wx, wy, ws);
+      spin.thin(wx, wy, ws);
+      z.Px = fma(-0.5, by, z.Px);
+      z.Py = fma(0.5, bx, z.Py);
+      return ok;
+    }
+    case K_RF: {     // A12, A13
+      double krf = e.krf_over_beta * ref.beta0;
+      double dE = e.volt * sin(fma(e.sign * krf, z.T, e.phi_s));
+      // E - E0' = p0c Pt + dE - dEs: the O(E0) terms are never formed
+      double num = fma(ref.p0c, z.Pt, dE - e.dEs);
+      if (e.dEs != 0.0) {
+        double p0_old = ref.p0c;
+        ref_set(ref, ref.E0 + e.dEs, ref.mass);
+        double sc = p0_old / ref.p0c;
+        z.Px *= sc; z.Py *= sc;
+      }
+      z.Pt = num / ref.p0c;
+      pcon_set(pc, z.Pt, ref, G);
+      return true;
+    }
+    case K_SNAKE:
+      spin.snake(Quat{e.qw, e.qx, e.qy, e.qs});
+      return true;
+    default: return true;
+  }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -719,56 +781,11 @@ __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_kernel(co
   PCon pc;
   pcon_set(pc, z.Pt, ref, a.G);
   bool alive = true;
+  FusedSpin<DEPTH> spin(z);
   for (long long turn = 0; turn < a.n_turns && alive; ++turn) {
     for (int ie = 0; ie < a.n_seq && alive; ++ie) {
       const DevElem& e = tab[seq[ie]];
-      switch (e.type) {
-        case K_DRIFT: alive = drift(z, e.L, pc, ref); break;
-        case K_SBEND:
-          if (SPLIT == SPLIT_DK) alive = sbend_teapot<DEPTH>(z, e, pc);
-          else alive = sbend_exact<DEPTH>(z, e, pc, ref);
-          break;
-        case K_QUAD:
-          if (SPLIT == SPLIT_MK) alive = quad_mk<DEPTH>(z, e, pc);
-          else alive = mult_dk<DEPTH>(z, e, pc, ref);
-          break;
-        case K_MULT: alive = mult_dk<DEPTH>(z, e, pc, ref); break;
-        case K_THIN: {   // A10: half kick, spin, half kick
-          double bx, by, wx, wy, ws;
-          mult_field(e, z.X, z.Y, bx, by);
-          z.Px = fma(-0.5, by, z.Px);
-          z.Py = fma(0.5, bx, z.Py);
-          double ps2 = 1.0 + pc.e0 - fma(z.Px, z.Px, z.Py * z.Py);
-          if (!(ps2 > 0.0)) { alive = false; break; }
-          omega_straight(1.0, z.Px, z.Py, rsqrt_nr(ps2), bx, by, pc, wx, wy, ws);
-          Quat q = quat_from_rotvec(wx, wy, ws);
-          quat_rotate(q, z.Sx, z.Sy, z.Ss);
-          z.Px = fma(-0.5, by, z.Px);
-          z.Py = fma(0.5, bx, z.Py);
-          break;
-        }
-        case K_RF: {     // A12, A13
-          double krf = e.krf_over_beta * ref.beta0;
-          double dE = e.volt * sin(fma(e.sign * krf, z.T, e.phi_s));
-          // E - E0' = p0c Pt + dE - dEs: the O(E0) terms are never formed
-          double num = fma(ref.p0c, z.Pt, dE - e.dEs);
-          if (e.dEs != 0.0) {
-            double p0_old = ref.p0c;
-            ref_set(ref, ref.E0 + e.dEs, ref.mass);
-            double sc = p0_old / ref.p0c;
-            z.Px *= sc; z.Py *= sc;
-          }
-          z.Pt = num / ref.p0c;
-          pcon_set(pc, z.Pt, ref, a.G);
-          break;
-        }
-        case K_SNAKE: {
-          Quat q{e.qw, e.qx, e.qy, e.qs};
-          quat_rotate(q, z.Sx, z.Sy, z.Ss);
-          break;
-        }
-        default: break;
-      }
+      alive = element_step<SPLIT>(z, e, pc, ref, a.G, spin);
     }
   }
   if (!alive) a.lost[j] = 1;

@@ -38,7 +38,8 @@ _dp = C.POINTER(C.c_double)
 
 EXPORTS = ["gst_lattice_create", "gst_lattice_destroy", "gst_lattice_steps_per_turn", "gst_bunch_init",
            "gst_bunch_destroy", "gst_track", "gst_polarization", "gst_emittance", "gst_bunch_lost",
-           "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host", "gst_fp64_peak", "gst_selftest_math", "gst_last_error"]
+           "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host", "gst_fp64_peak", "gst_selftest_math", "gst_last_error",
+           "gst_set_kernel_variant"]
 
 
 def lib():
@@ -70,6 +71,8 @@ def lib():
         L.gst_fp64_peak.argtypes = [_dp, _dp]
         L.gst_selftest_math.argtypes = [_dp]
         L.gst_selftest_math.restype = C.c_int
+        L.gst_set_kernel_variant.argtypes = [C.c_int]
+        L.gst_set_kernel_variant.restype = C.c_int
         for name in ("gst_lattice_create", "gst_bunch_init", "gst_track", "gst_polarization", "gst_emittance",
                      "gst_bunch_lost", "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host",
                      "gst_fp64_peak"):
@@ -208,6 +211,14 @@ class Bunch:
             self.close()
         except Exception:
             pass
+
+
+KERNEL_FUSED, KERNEL_PAIR = 0, 1
+
+
+def set_kernel_variant(variant):
+    """gst_set_kernel_variant: KERNEL_FUSED (default) or KERNEL_PAIR (experimental)."""
+    _check(lib().gst_set_kernel_variant(int(variant)))
 
 
 def fp64_peak():

@@ -196,6 +196,29 @@ def test_lost_particles_are_flagged_identically_and_excluded_from_reductions(gst
     assert np.max(np.abs(emit / O.emittance(ref, rlost) - 1)) < 1e-11
 
 
+@pytest.mark.parametrize("split,depth,n_slices", [(W.SPLIT_DRIFT_KICK, 1, 3), (W.SPLIT_BEND_KICK, 4, 8),
+                                                   (W.SPLIT_MATRIX_KICK, 3, 4), (W.SPLIT_BEND_KICK, 6, 32)])
+def test_pair_kernel_variant_is_bit_identical_to_the_fused_kernel(gst, split, depth, n_slices):
+    """GST_KERNEL_PAIR (two threads per particle, csrc/track_pair_kernel.cuh) runs the same arithmetic."""
+    lat = mixed_lattice(ramp=True)
+    bm = W.beam(12.0)
+    for n in (1, 33, 200):                       # one lane, a warp and a lane, several blocks with a ragged tail
+        st = W.gaussian_bunch(11, n, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
+        if n == 200:
+            st[1, 5] = 1.5                       # a lost particle (A15) in a warp that must keep in step
+        fused = gpu_track(gst, lat, bm, st, 3, split, n_slices, depth)
+        try:
+            gst.set_kernel_variant(gst.KERNEL_PAIR)
+            pair = gpu_track(gst, lat, bm, st, 3, split, n_slices, depth)
+        finally:
+            gst.set_kernel_variant(gst.KERNEL_FUSED)
+        assert np.array_equal(fused[1], pair[1])                 # lost flags
+        keep = ~fused[1].astype(bool)
+        assert np.array_equal(fused[0][:, keep], pair[0][:, keep])
+        assert np.array_equal(fused[2], pair[2])                 # polarization over the alive particles
+        assert fused[4] == pair[4]
+
+
 def test_chunked_tracking_is_bit_identical_to_one_call(gst):
     lat = mixed_lattice(ramp=True)
     bm = W.beam(12.0)
