@@ -50,10 +50,10 @@ struct DevTable {
 struct gst_lattice {
   std::vector<gst_element> elems;   // as given
   std::vector<gst_element> uniq;    // de-duplicated
-  std::vector<uint16_t> seq;        // index into uniq per lattice position
+  std::vector<uint32_t> seq;        // gst::seq_pack(index into uniq, type) per lattice position
   gst_beam beam;
   double C = 0;                     // circumference = sum of L
-  uint16_t* d_seq = nullptr;
+  uint32_t* d_seq = nullptr;
   mutable std::map<int, DevTable> tables;   // derived unique-element tables, keyed by n_slices
   mutable std::mutex mu;
   std::vector<double> cav_dEs;      // per cavity in lattice order: volt*sin(phi_s)
@@ -283,11 +283,11 @@ gst_status gst_lattice_create(const gst_element* elems, size_t n, const gst_beam
       if (k >= 65535) { delete lat; return fail(GST_EINVAL, "more than 65535 unique elements"); }
       lat->uniq.push_back(e);
     }
-    lat->seq[i] = (uint16_t)k;
+    lat->seq[i] = gst::seq_pack((uint32_t)k, e.type);
     if (e.type == GST_RFCAV) lat->cav_dEs.push_back(e.volt_eV * std::sin(e.phi_s));
   }
-  cudaError_t ce = cudaMalloc(&lat->d_seq, n * sizeof(uint16_t));
-  if (ce == cudaSuccess) ce = cudaMemcpy(lat->d_seq, lat->seq.data(), n * sizeof(uint16_t), cudaMemcpyHostToDevice);
+  cudaError_t ce = cudaMalloc(&lat->d_seq, n * sizeof(uint32_t));
+  if (ce == cudaSuccess) ce = cudaMemcpy(lat->d_seq, lat->seq.data(), n * sizeof(uint32_t), cudaMemcpyHostToDevice);
   if (ce != cudaSuccess) {
     if (lat->d_seq) cudaFree(lat->d_seq);
     delete lat;
@@ -387,7 +387,7 @@ gst_status gst_track(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, gst_
   a.mass = b->mass;
   a.G = lat->beam.G;
   size_t tab_bytes = lat->uniq.size() * sizeof(gst::DevElem);
-  size_t seq_bytes = (lat->seq.size() * sizeof(uint16_t) + 15) & ~size_t(15);
+  size_t seq_bytes = (lat->seq.size() * sizeof(uint32_t) + 15) & ~size_t(15);
   if (tab_bytes > 24 * 1024) return fail(GST_EINVAL, "too many unique elements for the shared-memory table (%zu)", lat->uniq.size());
   const bool pair = g_variant.load() == GST_KERNEL_PAIR;
   a.use_smem_seq = 0;

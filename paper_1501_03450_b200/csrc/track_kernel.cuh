@@ -59,7 +59,7 @@ struct TrackArgs {
   double* p[9];
   uint8_t* lost;
   const DevElem* tab;      // unique elements (global memory)
-  const uint16_t* seq;     // element sequence, indices into tab
+  const uint32_t* seq;     // element sequence: (index into tab) << 8 | type, see seq_pack()
   int n_unique;
   int n_seq;
   int use_smem_seq;
@@ -67,6 +67,10 @@ struct TrackArgs {
   long long n_turns;
   double E0, mass, G;
 };
+
+// One sequence entry carries the element type next to the table index, so that the per-element dispatch
+// needs one (prefetched) load instead of the chain seq -> table -> type.
+__host__ __device__ inline uint32_t seq_pack(uint32_t index, int type) { return (index << 8) | (uint32_t)type; }
 
 struct Quat { double w, x, y, s; };
 
@@ -215,11 +219,30 @@ __device__ __forceinline__ void quat_rotate(const Quat& q, double& Sx, double& S
 // Running products of the DEPTH trapezoid levels.  Level l has stride 2^l (l = 0 is the
 // finest); edge i belongs to it when 2^l | i.  The rotation for weight 2^l is obtained from the
 // finest one by angle doubling instead of a new sincos.
+// The Romberg table (39b) is linear in its first column, so its bottom-right entry is a fixed linear
+// combination of the DEPTH level products: row d-1 holds the weights of Q[0] (finest) .. Q[d-1] (coarsest),
+// obtained by running (39b) on unit vectors (exact integers over a common denominator).
+__constant__ double ROMBERG_W[6][6] = {
+    {1.0, 0.0, 0.0, 0.0, 0.0, 0.0},
+    {4.0 / 3.0, -1.0 / 3.0, 0.0, 0.0, 0.0, 0.0},
+    {64.0 / 45.0, -20.0 / 45.0, 1.0 / 45.0, 0.0, 0.0, 0.0},
+    {4096.0 / 2835.0, -1344.0 / 2835.0, 84.0 / 2835.0, -1.0 / 2835.0, 0.0, 0.0},
+    {1048576.0 / 722925.0, -348160.0 / 722925.0, 22848.0 / 722925.0, -340.0 / 722925.0, 1.0 / 722925.0, 0.0},
+    {1073741824.0 / 739552275.0, -357564416.0 / 739552275.0, 23744512.0 / 739552275.0, -371008.0 / 739552275.0,
+     1364.0 / 739552275.0, -1.0 / 739552275.0}};
+
 template <int DEPTH> struct SpinAcc {
   Quat Q[DEPTH];
-  __device__ __forceinline__ void reset() {
+  // first edge of an element: every level starts from its own rotation (the product with the identity
+  // is skipped; bit-identical apart from the sign of a zero)
+  __device__ __forceinline__ void init(double wx, double wy, double ws) {
+    Quat q = quat_from_rotvec(wx, wy, ws);
+    Q[0] = q;
 #pragma unroll
-    for (int l = 0; l < DEPTH; ++l) Q[l] = Quat{1.0, 0.0, 0.0, 0.0};
+    for (int l = 1; l < DEPTH; ++l) {
+      q = quat_double(q);
+      Q[l] = q;
+    }
   }
   // fold rotation vector (weight * ds * Omega_i) into levels 0..NS-1, all known at compile time
   template <int NS>
@@ -243,23 +266,17 @@ template <int DEPTH> struct SpinAcc {
       Q[l] = quat_mul(q, Q[l]);
     }
   }
-  // Romberg limit (39b) P:542 of the level products, normalised, applied to S (a11)
+  // Romberg limit (39b) P:542 of the level products, normalised, applied to S (a11).
+  // Q[l] holds step h*2^l, i.e. column entry k = DEPTH-1-l of (38).
   __device__ __forceinline__ void finish(double& Sx, double& Sy, double& Ss) {
-    // Q[l] holds step h*2^l, i.e. column entry k = DEPTH-1-l of (38).  Run the table in place.
-    double f = 1.0;
+    Quat q;
+    q.w = ROMBERG_W[DEPTH - 1][0] * Q[0].w; q.x = ROMBERG_W[DEPTH - 1][0] * Q[0].x;
+    q.y = ROMBERG_W[DEPTH - 1][0] * Q[0].y; q.s = ROMBERG_W[DEPTH - 1][0] * Q[0].s;
 #pragma unroll
-    for (int j = 1; j < DEPTH; ++j) {
-      f *= 4.0;
-      const double c1 = f / (f - 1.0), c2 = 1.0 / (f - 1.0);
-#pragma unroll
-      for (int l = 0; l + j < DEPTH; ++l) {        // finer entry Q[l], coarser Q[l+1]
-        Q[l].w = fma(c1, Q[l].w, -c2 * Q[l + 1].w);
-        Q[l].x = fma(c1, Q[l].x, -c2 * Q[l + 1].x);
-        Q[l].y = fma(c1, Q[l].y, -c2 * Q[l + 1].y);
-        Q[l].s = fma(c1, Q[l].s, -c2 * Q[l + 1].s);
-      }
+    for (int l = 1; l < DEPTH; ++l) {
+      q.w = fma(ROMBERG_W[DEPTH - 1][l], Q[l].w, q.w); q.x = fma(ROMBERG_W[DEPTH - 1][l], Q[l].x, q.x);
+      q.y = fma(ROMBERG_W[DEPTH - 1][l], Q[l].y, q.y); q.s = fma(ROMBERG_W[DEPTH - 1][l], Q[l].s, q.s);
     }
-    Quat q = Q[0];
     double n2 = fma(q.w, q.w, fma(q.x, q.x, fma(q.y, q.y, q.s * q.s)));
     double rn = rsqrt_nr(n2);
     q.w *= rn; q.x *= rn; q.y *= rn; q.s *= rn;
@@ -304,31 +321,37 @@ template <int DEPTH> struct FusedSpin {
   template <class Stepper>
   __device__ __forceinline__ void run(Stepper& s, int N, double ds) {
     SpinAcc<DEPTH> acc;
-    acc.reset();
     const double hds = 0.5 * ds;
     double wx, wy, ws;
     s.omega(hds, wx, wy, ws);                       // pending edge 0, half weight
+    s.advance();                                    // orbit slice 1 ...
+    acc.init(wx, wy, ws);                           // ... independent of the spin work of edge 0
     if (DEPTH == 1) {
-      for (int i = 1; i <= N; ++i) {
-        s.advance();                                // orbit slice i ...
-        acc.template fold_static<1>(wx, wy, ws);    // ... independent of the spin work of edge i-1
+      s.omega(N == 1 ? hds : ds, wx, wy, ws);
+      for (int i = 2; i <= N; ++i) {
+        s.advance();                                // slice i next to the fold of edge i-1
+        acc.template fold_static<1>(wx, wy, ws);
         s.omega(i == N ? hds : ds, wx, wy, ws);
       }
       acc.template fold_static<1>(wx, wy, ws);
     } else {
-      // DEPTH >= 2: N is even (A4).  Edges are taken in pairs (even, odd): the odd edge belongs to
+      // DEPTH >= 2: N is even (A4).  Edges are taken in pairs (odd, even): the odd edge belongs to
       // level 0 only, the even edge to levels 0 and 1 and, where 4 | i, 8 | i, ..., to higher ones.
-      for (int i = 0; i < N; i += 2) {
-        s.advance();
+      s.omega(ds, wx, wy, ws);                                 // pending edge 1
+      for (int i = 1; i + 1 < N; i += 2) {
+        s.advance();                                           // slice i+1
+        acc.template fold_static<1>(wx, wy, ws);               // odd edge i
+        s.omega(ds, wx, wy, ws);
+        s.advance();                                           // slice i+2
         {
-          Quat q = acc.template fold_static<2>(wx, wy, ws);    // even edge i
-          acc.template fold_dynamic<2>(i, q);
+          Quat q = acc.template fold_static<2>(wx, wy, ws);    // even edge i+1
+          acc.template fold_dynamic<2>(i + 1, q);
         }
         s.omega(ds, wx, wy, ws);
-        s.advance();
-        acc.template fold_static<1>(wx, wy, ws);               // odd edge i+1
-        s.omega(i + 2 == N ? hds : ds, wx, wy, ws);
       }
+      s.advance();                                             // slice N
+      acc.template fold_static<1>(wx, wy, ws);                 // odd edge N-1
+      s.omega(hds, wx, wy, ws);
       acc.template fold_static<DEPTH>(wx, wy, ws);             // edge N: every level (2^(DEPTH-1) | N)
     }
     acc.finish(Sx, Sy, Ss);
@@ -694,52 +717,51 @@ __device__ __forceinline__ bool quad_mk(State& z, const DevElem& e, const PCon& 
 }
 
 // ---------------------------------------------------------------------------------------------
-// one element (the switch is uniform across the grid: every particle is in the same element)
+// one element (the dispatch is uniform across the grid: every particle is in the same element)
 // ---------------------------------------------------------------------------------------------
+// The tests are ordered by how often each type occurs in a ring (drifts, quadrupoles, bends, thin lenses).
 template <int SPLIT, class Spin>
-__device__ __forceinline__ bool element_step(State& z, const DevElem& e, PCon& pc, Ref& ref, double G, Spin& spin) {
-  switch (e.type) {
-    case K_DRIFT: return drift(z, e.L, pc, ref);
-    case K_SBEND:
-      if (SPLIT == SPLIT_DK) return sbend_teapot(z, e, pc, spin);
-      return sbend_exact(z, e, pc, ref, spin);
-    case K_QUAD:
-      if (SPLIT == SPLIT_MK) return quad_mk(z, e, pc, spin);
-      return mult_dk(z, e, pc, ref, spin);
-    case K_MULT: return mult_dk(z, e, pc, ref, spin);
-    case K_THIN: {   // A10: half kick, spin, half kick
-      double bx, by, wx, wy, ws;
-      mult_field(e, z.X, z.Y, bx, by);
-      z.Px = fma(-0.5, by, z.Px);
-      z.Py = fma(0.5, bx, z.Py);
-      const double ps2 = 1.0 + pc.e0 - fma(z.Px, z.Px, z.Py * z.Py);
-      const bool ok = ps2 > 0.0;
-      omega_straight(1.0, z.Px, z.Py, rsqrt_nr(ok ? ps2 : 1.0), bx, by, pc, wx, wy, ws);
-      spin.thin(wx, wy, ws);
-      z.Px = fma(-0.5, by, z.Px);
-      z.Py = fma(0.5, bx, z.Py);
-      return ok;
-    }
-    case K_RF: {     // A12, A13
-      double krf = e.krf_over_beta * ref.beta0;
-      double dE = e.volt * sin(fma(e.sign * krf, z.T, e.phi_s));
-      // E - E0' = p0c Pt + dE - dEs: the O(E0) terms are never formed
-      double num = fma(ref.p0c, z.Pt, dE - e.dEs);
-      if (e.dEs != 0.0) {
-        double p0_old = ref.p0c;
-        ref_set(ref, ref.E0 + e.dEs, ref.mass);
-        double sc = p0_old / ref.p0c;
-        z.Px *= sc; z.Py *= sc;
-      }
-      z.Pt = num / ref.p0c;
-      pcon_set(pc, z.Pt, ref, G);
-      return true;
-    }
-    case K_SNAKE:
-      spin.snake(Quat{e.qw, e.qx, e.qy, e.qs});
-      return true;
-    default: return true;
+__device__ __forceinline__ bool element_step(int type, State& z, const DevElem& e, PCon& pc, Ref& ref, double G, Spin& spin) {
+  if (type == K_DRIFT) return drift(z, e.L, pc, ref);
+  if (type == K_QUAD) {
+    if (SPLIT == SPLIT_MK) return quad_mk(z, e, pc, spin);
+    return mult_dk(z, e, pc, ref, spin);
   }
+  if (type == K_SBEND) {
+    if (SPLIT == SPLIT_DK) return sbend_teapot(z, e, pc, spin);
+    return sbend_exact(z, e, pc, ref, spin);
+  }
+  if (type == K_THIN) {   // A10: half kick, spin, half kick
+    double bx, by, wx, wy, ws;
+    mult_field(e, z.X, z.Y, bx, by);
+    z.Px = fma(-0.5, by, z.Px);
+    z.Py = fma(0.5, bx, z.Py);
+    const double ps2 = 1.0 + pc.e0 - fma(z.Px, z.Px, z.Py * z.Py);
+    const bool ok = ps2 > 0.0;
+    omega_straight(1.0, z.Px, z.Py, rsqrt_nr(ok ? ps2 : 1.0), bx, by, pc, wx, wy, ws);
+    spin.thin(wx, wy, ws);
+    z.Px = fma(-0.5, by, z.Px);
+    z.Py = fma(0.5, bx, z.Py);
+    return ok;
+  }
+  if (type == K_MULT) return mult_dk(z, e, pc, ref, spin);
+  if (type == K_RF) {     // A12, A13
+    double krf = e.krf_over_beta * ref.beta0;
+    double dE = e.volt * sin(fma(e.sign * krf, z.T, e.phi_s));
+    // E - E0' = p0c Pt + dE - dEs: the O(E0) terms are never formed
+    double num = fma(ref.p0c, z.Pt, dE - e.dEs);
+    if (e.dEs != 0.0) {
+      double p0_old = ref.p0c;
+      ref_set(ref, ref.E0 + e.dEs, ref.mass);
+      double sc = p0_old / ref.p0c;
+      z.Px *= sc; z.Py *= sc;
+    }
+    z.Pt = num / ref.p0c;
+    pcon_set(pc, z.Pt, ref, G);
+    return true;
+  }
+  if (type == K_SNAKE) spin.snake(Quat{e.qw, e.qx, e.qy, e.qs});
+  return true;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -757,14 +779,14 @@ template <int SPLIT, int DEPTH>
 __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_kernel(const TrackArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   DevElem* tab = reinterpret_cast<DevElem*>(smem_raw);
-  const uint16_t* seq = a.seq;
+  const uint32_t* seq = a.seq;
   {   // a0: stage the unique-element table (and the sequence when it fits) into shared memory
     const int nw = a.n_unique * (int)(sizeof(DevElem) / sizeof(double));
     const double* src = reinterpret_cast<const double*>(a.tab);
     double* dst = reinterpret_cast<double*>(smem_raw);
     for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
     if (a.use_smem_seq) {
-      uint16_t* sseq = reinterpret_cast<uint16_t*>(smem_raw + (size_t)a.n_unique * sizeof(DevElem));
+      uint32_t* sseq = reinterpret_cast<uint32_t*>(smem_raw + (size_t)a.n_unique * sizeof(DevElem));
       for (int i = threadIdx.x; i < a.n_seq; i += blockDim.x) sseq[i] = a.seq[i];
       seq = sseq;
     }
@@ -780,15 +802,27 @@ __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_kernel(co
   ref_set(ref, a.E0, a.mass);
   PCon pc;
   pcon_set(pc, z.Pt, ref, a.G);
-  bool alive = true;
+  // The turn and element loops run to the end for every thread, so that their counters, the sequence
+  // loads and the type dispatch are warp-uniform (uniform registers, no divergence bookkeeping); a
+  // particle that is lost (A15) goes on with the reference orbit and nothing of it is stored.
+  bool lost = false;
   FusedSpin<DEPTH> spin(z);
-  for (long long turn = 0; turn < a.n_turns && alive; ++turn) {
-    for (int ie = 0; ie < a.n_seq && alive; ++ie) {
-      const DevElem& e = tab[seq[ie]];
-      alive = element_step<SPLIT>(z, e, pc, ref, a.G, spin);
+  uint32_t nxt = seq[0];
+  for (long long turn = 0; turn < a.n_turns; ++turn) {
+#pragma unroll 1
+    for (int ie = 0; ie < a.n_seq; ++ie) {
+      const uint32_t cur = nxt;
+      nxt = seq[ie + 1 < a.n_seq ? ie + 1 : 0];          // next element's entry, one element ahead
+      const DevElem& e = tab[cur >> 8];
+      const bool ok = element_step<SPLIT>((int)(cur & 0xffu), z, e, pc, ref, a.G, spin);
+      if (!ok) {
+        lost = true;
+        z.X = z.Px = z.Y = z.Py = z.T = z.Pt = 0.0;
+        pcon_set(pc, 0.0, ref, a.G);
+      }
     }
   }
-  if (!alive) a.lost[j] = 1;
+  if (lost) { a.lost[j] = 1; return; }
   a.p[0][j] = z.X; a.p[1][j] = z.Px; a.p[2][j] = z.Y; a.p[3][j] = z.Py; a.p[4][j] = z.T; a.p[5][j] = z.Pt;
   a.p[6][j] = z.Sx; a.p[7][j] = z.Sy; a.p[8][j] = z.Ss;
 }

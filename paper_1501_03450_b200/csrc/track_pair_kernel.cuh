@@ -113,9 +113,14 @@ struct PopSpin {
   template <int DEPTH>
   __device__ __forceinline__ void thick(int N, double& Sx, double& Sy, double& Ss) {
     SpinAcc<DEPTH> acc;
-    acc.reset();
+    {
+      Quat q = pop();                               // edge 0 starts every level
+      acc.Q[0] = q;
+#pragma unroll
+      for (int l = 1; l < DEPTH; ++l) { q = quat_double(q); acc.Q[l] = q; }
+    }
 #pragma unroll 1
-    for (int i = 0; i <= N; ++i) {
+    for (int i = 1; i <= N; ++i) {
       Quat q = pop();
       acc.Q[0] = quat_mul(q, acc.Q[0]);
       acc.template fold_dynamic<1>(i, q);
@@ -134,7 +139,7 @@ template <int DEPTH> struct PairCfg {
 
 // ---- the two roles ---------------------------------------------------------------------------
 template <int SPLIT>
-__device__ __forceinline__ void orbit_role(const TrackArgs& a, const DevElem* tab, const uint16_t* seq, double* ring_lane,
+__device__ __forceinline__ void orbit_role(const TrackArgs& a, const DevElem* tab, const uint32_t* seq, double* ring_lane,
                                            uint8_t* flag_lane, long long j, bool valid) {
   Chan ch{ring_lane, 0};
   State z;
@@ -152,8 +157,9 @@ __device__ __forceinline__ void orbit_role(const TrackArgs& a, const DevElem* ta
   for (long long turn = 0; turn < a.n_turns; ++turn) {
 #pragma unroll 1
     for (int ie = 0; ie < a.n_seq; ++ie) {
-      const DevElem& e = tab[seq[ie]];
-      const bool ok = element_step<SPLIT>(z, e, pc, ref, a.G, spin);
+      const uint32_t cur = seq[ie];
+      const DevElem& e = tab[cur >> 8];
+      const bool ok = element_step<SPLIT>((int)(cur & 0xffu), z, e, pc, ref, a.G, spin);
       if (!ok) {
         // A15: the particle is lost.  The warp must stay in step with its partner, so the lane goes on
         // with the reference orbit (all zeros); nothing of it is stored.
@@ -175,7 +181,7 @@ __device__ __forceinline__ void orbit_role(const TrackArgs& a, const DevElem* ta
 }
 
 template <int DEPTH>
-__device__ __forceinline__ void spin_role(const TrackArgs& a, const DevElem* tab, const uint16_t* seq, double* ring_lane,
+__device__ __forceinline__ void spin_role(const TrackArgs& a, const DevElem* tab, const uint32_t* seq, double* ring_lane,
                                           long long j, bool valid, double& Sx, double& Sy, double& Ss) {
   Chan ch{ring_lane, 0};
   if (valid) { Sx = a.p[6][j]; Sy = a.p[7][j]; Ss = a.p[8][j]; }
@@ -184,8 +190,9 @@ __device__ __forceinline__ void spin_role(const TrackArgs& a, const DevElem* tab
   for (long long turn = 0; turn < a.n_turns; ++turn) {
 #pragma unroll 1
     for (int ie = 0; ie < a.n_seq; ++ie) {
-      const DevElem& e = tab[seq[ie]];
-      const int type = e.type;
+      const uint32_t cur = seq[ie];
+      const DevElem& e = tab[cur >> 8];
+      const int type = (int)(cur & 0xffu);
       if (type == K_SBEND || type == K_QUAD || type == K_MULT) {
         spin.template thick<DEPTH>(e.N, Sx, Sy, Ss);
       } else if (type == K_THIN) {
@@ -209,14 +216,14 @@ __global__ void __launch_bounds__(PairCfg<DEPTH>::THREADS, PairCfg<DEPTH>::MIN_B
   uint8_t* flag = smem_raw + PAIRS * PAIR_RING_BYTES;
   unsigned char* tab_raw = flag + PAIRS * 32;
   DevElem* tab = reinterpret_cast<DevElem*>(tab_raw);
-  const uint16_t* seq = a.seq;
+  const uint32_t* seq = a.seq;
   {
     const int nw = a.n_unique * (int)(sizeof(DevElem) / sizeof(double));
     const double* src = reinterpret_cast<const double*>(a.tab);
     double* dst = reinterpret_cast<double*>(tab_raw);
     for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
     if (a.use_smem_seq) {
-      uint16_t* sseq = reinterpret_cast<uint16_t*>(tab_raw + (size_t)a.n_unique * sizeof(DevElem));
+      uint32_t* sseq = reinterpret_cast<uint32_t*>(tab_raw + (size_t)a.n_unique * sizeof(DevElem));
       for (int i = threadIdx.x; i < a.n_seq; i += blockDim.x) sseq[i] = a.seq[i];
       seq = sseq;
     }
