@@ -515,7 +515,7 @@ gst_status gst_selftest_math(double out[2]) {
   return GST_OK;
 }
 
-gst_status gst_fp64_peak(double* out_tflops, double* out_ms) {
+static gst_status fp64_peak_impl(bool three_registers, double* out_tflops, double* out_ms) {
   if (!out_tflops) return fail(GST_EINVAL, "null argument");
   int dev = 0, sms = 0;
   CUDA_TRY(cudaGetDevice(&dev));
@@ -529,7 +529,8 @@ gst_status gst_fp64_peak(double* out_tflops, double* out_ms) {
   float best = 1e30f;
   for (int rep = 0; rep < 6; ++rep) {
     cudaEventRecord(e0);
-    gst::dfma_peak_kernel<<<sms * 8, gst::PEAK_BLOCK>>>(d_out, iters, 1.0 + 1e-9 * rep);
+    if (three_registers) gst::dfma_rrr_kernel<<<sms * 8, gst::PEAK_BLOCK>>>(d_out, iters, 1.0 + 1e-9 * rep);
+    else gst::dfma_peak_kernel<<<sms * 8, gst::PEAK_BLOCK>>>(d_out, iters, 1.0 + 1e-9 * rep);
     cudaEventRecord(e1);
     CUDA_TRY(cudaEventSynchronize(e1));
     float ms = 0;
@@ -545,5 +546,8 @@ gst_status gst_fp64_peak(double* out_tflops, double* out_ms) {
   if (out_ms) *out_ms = best;
   return GST_OK;
 }
+
+gst_status gst_fp64_peak(double* out_tflops, double* out_ms) { return fp64_peak_impl(false, out_tflops, out_ms); }
+gst_status gst_fp64_peak_rrr(double* out_tflops, double* out_ms) { return fp64_peak_impl(true, out_tflops, out_ms); }
 
 }  // extern "C"

@@ -39,7 +39,7 @@ _dp = C.POINTER(C.c_double)
 EXPORTS = ["gst_lattice_create", "gst_lattice_destroy", "gst_lattice_steps_per_turn", "gst_bunch_init",
            "gst_bunch_destroy", "gst_track", "gst_polarization", "gst_emittance", "gst_bunch_lost",
            "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host", "gst_fp64_peak", "gst_selftest_math", "gst_last_error",
-           "gst_set_kernel_variant"]
+           "gst_set_kernel_variant", "gst_fp64_peak_rrr"]
 
 
 def lib():
@@ -69,6 +69,8 @@ def lib():
         L.gst_track_host.argtypes = [vp, C.POINTER(_dp), C.c_size_t, C.c_int64, C.c_int, C.c_int, C.c_int, _dp,
                                      C.POINTER(C.c_int64)]
         L.gst_fp64_peak.argtypes = [_dp, _dp]
+        L.gst_fp64_peak_rrr.argtypes = [_dp, _dp]
+        L.gst_fp64_peak_rrr.restype = C.c_int
         L.gst_selftest_math.argtypes = [_dp]
         L.gst_selftest_math.restype = C.c_int
         L.gst_set_kernel_variant.argtypes = [C.c_int]
@@ -226,6 +228,14 @@ def fp64_peak():
     t = C.c_double(0)
     ms = C.c_double(0)
     _check(lib().gst_fp64_peak(C.byref(t), C.byref(ms)))
+    return t.value, ms.value
+
+
+def fp64_peak_rrr():
+    """gst_fp64_peak_rrr: the same with three distinct register operands per DFMA (TFLOP/s, ms)."""
+    t = C.c_double(0)
+    ms = C.c_double(0)
+    _check(lib().gst_fp64_peak_rrr(C.byref(t), C.byref(ms)))
     return t.value, ms.value
 
 
