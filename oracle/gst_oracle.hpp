@@ -34,7 +34,11 @@ namespace orc {
 // element table entry (the oracle's own definition; field meaning identical to DESIGN.md §2)
 // ----------------------------------------------------------------------------------------------
 enum ElemType { DRIFT = 0, SBEND = 1, QUAD = 2, MULTIPOLE = 3, THINMULT = 4, RFCAV = 5, SNAKE = 6, MARKER = 7 };
-enum Split { SPLIT_DRIFT_KICK = 0, SPLIT_BEND_KICK = 1, SPLIT_MATRIX_KICK = 2 };
+enum Split { SPLIT_DRIFT_KICK = 0, SPLIT_BEND_KICK = 1, SPLIT_MATRIX_KICK = 2,
+             // the same splits with every second-order slice map (27) replaced by the fourth-order symmetric
+             // composition of three of them ("more sophisticated symmetric compositions", "higher-order
+             // versions of (27)", refs [62, 45, 23]); reading R5
+             SPLIT_DRIFT_KICK_4 = 3, SPLIT_BEND_KICK_4 = 4, SPLIT_MATRIX_KICK_4 = 5 };
 
 struct Element {
   int32_t type;
@@ -365,8 +369,8 @@ template <class R> Vec3<R> element_field(const Element& e, const Orbit<R>& z) {
   return Vec3<R>{bx, by, R(0)};
 }
 
-// one orbital slice of a thick magnet of the given type with the given split (A16)
-template <class R> bool orbit_slice(Orbit<R>& z, const Element& e, R ds, int split, const Reference<R>& ref) {
+// one second-order orbital slice of a thick magnet of the given type with the given split (A16)
+template <class R> bool orbit_slice2(Orbit<R>& z, const Element& e, R ds, int split, const Reference<R>& ref) {
   if (e.type == SBEND) {
     if (split == SPLIT_DRIFT_KICK) {                                 // TEAPOT (30),(31), composed as (27)
       if (!curved_drift(z, ds / R(2), R(e.h), ref)) return false;
@@ -384,6 +388,25 @@ template <class R> bool orbit_slice(Orbit<R>& z, const Element& e, R ds, int spl
   if (!drift(z, ds / R(2), ref)) return false;
   multipole_kick(z, ds, e.kn, e.ks);
   return drift(z, ds / R(2), ref);
+}
+
+// is the slice map of this element exact under this split?  (an exact flow needs no composition)
+inline bool slice_is_exact(const Element& e, int base_split) { return e.type == SBEND && base_split != SPLIT_DRIFT_KICK; }
+
+// one orbital slice: second order (27), or the fourth-order symmetric composition
+//   S4(ds) = S2(x1 ds) S2(x0 ds) S2(x1 ds),  x1 = 1/(2 - 2^(1/3)),  x0 = 1 - 2 x1 = -2^(1/3) x1
+// (the triple-jump composition of refs [62, 23]: x0 + 2 x1 = 1 keeps the length, x0^3 + 2 x1^3 = 0 cancels
+// the third-order error term of the symmetric S2).  The middle step runs backwards (x0 < 0).
+template <class R> bool orbit_slice(Orbit<R>& z, const Element& e, R ds, int split, const Reference<R>& ref) {
+  const int base = split % 3;
+  if (split < 3 || slice_is_exact(e, base)) return orbit_slice2(z, e, ds, base, ref);
+  R cbrt2 = R(1.2599210498948732);                                    // 2^(1/3), polished by Newton to the precision of R
+  for (int it = 0; it < 3; ++it) cbrt2 = cbrt2 - (cbrt2 * cbrt2 * cbrt2 - R(2)) / (R(3) * cbrt2 * cbrt2);
+  const R x1 = R(1) / (R(2) - cbrt2);
+  const R x0 = R(1) - R(2) * x1;
+  if (!orbit_slice2(z, e, x1 * ds, base, ref)) return false;
+  if (!orbit_slice2(z, e, x0 * ds, base, ref)) return false;
+  return orbit_slice2(z, e, x1 * ds, base, ref);
 }
 
 // returns false if the particle is lost inside this element (A15): p is then restored to its

@@ -48,7 +48,7 @@ template <class R> double reference_after(const Element* el, size_t n_el, const 
 }
 
 int validate(const Element* el, size_t n_el, int split, int n_slices, int depth) {
-  if (n_slices < 1 || depth < 1 || depth > 12 || split < 0 || split > 2) return 1;
+  if (n_slices < 1 || depth < 1 || depth > 12 || split < 0 || split > 5) return 1;
   for (size_t e = 0; e < n_el; ++e) {
     int t = el[e].type;
     if (t < 0 || t > MARKER) return 1;

@@ -1,0 +1,160 @@
+"""The two BASELINE studies that are more than one timed launch, run through the C ABI on one GPU.
+
+    python -m paper_1501_03450_b200.studies ramp  [--particles N] [--turns T] [--chunk 100] [--out FILE.md]
+    python -m paper_1501_03450_b200.studies sweep [--particles N] [--turns T] [--out FILE.md]
+
+ramp  : BASELINE configs[3] (SURVEY config 4): the RHIC-like ring with its cavity ramping the energy by
+        100 keV/turn from G*gamma = 45.0, 2^20 particles, 5000 turns; the bunch polarization, emittances
+        and lost count are reported every `chunk` turns (gst_track in chunks + gst_polarization, the
+        checkpoint pattern of P:776).
+sweep : BASELINE configs[4] (SURVEY config 5): accuracy vs throughput on the ring without snakes,
+        262 144 particles, 100 turns, for the three splits x the 27 valid (slices, depth) pairs (reading A4).
+        Errors are the paper's (44) P:622 and (46) P:733 against a reference by refinement, as the paper
+        does: matrix-kick, 128 slices, depth 6 -- computed by the same library; that this
+        reference equals the CPU oracle's is what tests/test_gpu_parity.py::test_config5_reference_run checks.
+
+Every number of the hot path comes from the CUDA kernels; torch is used for device memory, the error
+norms of the report and nothing else.  One JSON line per report row on stdout; --out adds a markdown table.
+"""
+import argparse
+import json
+import sys
+import time
+
+import numpy as np
+
+from . import workloads as W
+
+G_PROTON = 1.792847
+
+
+def _device_state(torch, state):
+    return torch.tensor(state, dtype=torch.float64, device="cuda").contiguous()
+
+
+def _timed_track(torch, bunch, lat, turns, split, n_slices, depth):
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    bunch.track(lat, turns, split, n_slices, depth)
+    e1.record()
+    e1.synchronize()
+    return e0.elapsed_time(e1)
+
+
+def ramp(args):
+    import torch
+    from . import gst
+    cfg = W.config(4, n_particles=args.particles, n_turns=args.turns)
+    n, turns = cfg["state"].shape[1], cfg["n_turns"]
+    lat = gst.Lattice(cfg["lattice"], cfg["beam"])
+    spt = lat.steps_per_turn(cfg["n_slices"])
+    dev = _device_state(torch, cfg["state"])
+    bunch = gst.Bunch(dev)
+    rows, ms_total, done = [], 0.0, 0
+    pol, lost = bunch.polarization()
+    ex, ey = bunch.emittance()
+    g0 = cfg["beam"]["gamma0"]
+    bg0 = float(np.sqrt(g0 * g0 - 1.0))
+    rows.append(dict(turn=0, G_gamma=G_PROTON * g0, P=[float(x) for x in pol], eps_n=[ex * bg0, ey * bg0], lost=int(lost)))
+    print(json.dumps(rows[-1]))
+    while done < turns:
+        nt = min(args.chunk, turns - done)
+        ms_total += _timed_track(torch, bunch, lat, nt, cfg["split"], cfg["n_slices"], cfg["depth"])
+        done += nt
+        pol, lost = bunch.polarization()
+        ex, ey = bunch.emittance()
+        g, turn = bunch.reference()
+        bg = float(np.sqrt(g * g - 1.0))
+        # normalised rms emittance beta*gamma*eps: constant under adiabatic damping (A13)
+        rows.append(dict(turn=int(turn), G_gamma=G_PROTON * g, P=[float(x) for x in pol], eps_n=[ex * bg, ey * bg],
+                         lost=int(lost)))
+        print(json.dumps(rows[-1]))
+        sys.stdout.flush()
+    rate = float(n) * turns * spt / (ms_total * 1e-3)
+    summary = dict(study="ramp", particles=n, turns=turns, chunk=args.chunk, steps_per_turn=spt,
+                   track_ms=ms_total, steps_per_s=rate, split=W.SPLIT_NAMES[cfg["split"]],
+                   n_slices=cfg["n_slices"], depth=cfg["depth"])
+    print(json.dumps(summary))
+    if args.out:
+        with open(args.out, "w") as f:
+            f.write("# Ramp through G*gamma = 45.0 -> %.3f (config 4), %d particles, %d turns\n\n" % (rows[-1]["G_gamma"], n, turns))
+            f.write("Command: `python -m paper_1501_03450_b200.studies ramp --particles %d --turns %d --chunk %d`\n\n" % (n, turns, args.chunk))
+            f.write("track kernel time %.1f s, %.4g particle-element-steps/s\n\n" % (ms_total * 1e-3, rate))
+            f.write("| turn | G*gamma | Px | Py | Ps | |P| | eps_n,x [m] | eps_n,y [m] | lost |\n|---|---|---|---|---|---|---|---|---|\n")
+            for r in rows:
+                f.write("| %d | %.5f | %+.6f | %+.6f | %+.6f | %.6f | %.4e | %.4e | %d |\n"
+                        % (r["turn"], r["G_gamma"], r["P"][0], r["P"][1], r["P"][2], r["P"][3], r["eps_n"][0], r["eps_n"][1], r["lost"]))
+    bunch.close()
+    lat.close()
+
+
+def sweep(args):
+    import torch
+    from . import gst
+    cfg = W.config(5, n_particles=args.particles, n_turns=args.turns)
+    n, turns = cfg["state"].shape[1], cfg["n_turns"]
+    lat = gst.Lattice(cfg["lattice"], cfg["beam"])
+    init = _device_state(torch, cfg["state"])
+
+    def run(split, n_slices, depth):
+        dev = init.clone()
+        b = gst.Bunch(dev)
+        ms = _timed_track(torch, b, lat, turns, split, n_slices, depth)
+        _, lost = b.polarization()
+        b.close()
+        return dev, ms, int(lost)
+
+    ref, ref_ms, ref_lost = run(W.SPLIT_MATRIX_KICK, args.ref_slices, 6)
+    print(json.dumps(dict(study="sweep", reference=dict(split="matrix_kick", n_slices=args.ref_slices, depth=6, ms=ref_ms,
+                                                        lost=ref_lost), particles=n, turns=turns)))
+    rows = []
+    for split in (W.SPLIT_DRIFT_KICK, W.SPLIT_BEND_KICK, W.SPLIT_MATRIX_KICK):
+        for n_slices, depth in W.sweep_pairs():
+            if n_slices > args.max_slices:
+                continue
+            dev, ms, lost = run(split, n_slices, depth)
+            dS = torch.linalg.vector_norm(dev[6:9] - ref[6:9], dim=0).mean().item()          # (46) P:733
+            dX = torch.sqrt(torch.mean((dev[0] - ref[0]) ** 2)).item()                          # (44) P:622
+            spt = lat.steps_per_turn(n_slices)
+            row = dict(split=W.SPLIT_NAMES[split], n_slices=n_slices, depth=depth, spin_err=dS, x_rms_err=dX,
+                       ms=ms, steps_per_s=float(n) * turns * spt / (ms * 1e-3),
+                       particle_turns_per_s=float(n) * turns / (ms * 1e-3), lost=lost)
+            rows.append(row)
+            print(json.dumps(row))
+            sys.stdout.flush()
+            del dev
+    if args.out:
+        with open(args.out, "w") as f:
+            f.write("# Accuracy vs throughput (config 5): RHIC-like ring without snakes, %d particles, %d turns\n\n" % (n, turns))
+            f.write("Command: `python -m paper_1501_03450_b200.studies sweep --particles %d --turns %d`\n\n" % (n, turns))
+            f.write("Reference: matrix-kick, %d slices, depth 6 (%.1f s).  spin error = (46) P:733, X error = (44) P:622.\n\n"
+                    % (args.ref_slices, ref_ms * 1e-3))
+            f.write("| split | slices | depth | spin error | rms X error [m] | steps/s | particle-turns/s |\n|---|---|---|---|---|---|---|\n")
+            for r in rows:
+                f.write("| %s | %d | %d | %.3e | %.3e | %.4g | %.4g |\n" % (r["split"], r["n_slices"], r["depth"], r["spin_err"],
+                                                                       r["x_rms_err"], r["steps_per_s"], r["particle_turns_per_s"]))
+    lat.close()
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
+    sub = ap.add_subparsers(dest="study", required=True)
+    r = sub.add_parser("ramp")
+    r.add_argument("--particles", type=int, default=None)
+    r.add_argument("--turns", type=int, default=None)
+    r.add_argument("--chunk", type=int, default=100)
+    r.add_argument("--out", default=None)
+    s = sub.add_parser("sweep")
+    s.add_argument("--particles", type=int, default=None)
+    s.add_argument("--turns", type=int, default=None)
+    s.add_argument("--ref-slices", type=int, default=128)
+    s.add_argument("--max-slices", type=int, default=64)
+    s.add_argument("--out", default=None)
+    args = ap.parse_args(argv)
+    t0 = time.time()
+    (ramp if args.study == "ramp" else sweep)(args)
+    print(json.dumps(dict(wall_s=time.time() - t0)))
+
+
+if __name__ == "__main__":
+    main()

@@ -17,7 +17,10 @@ import numpy as np
 
 DRIFT, SBEND, QUAD, MULTIPOLE, THINMULT, RFCAV, SNAKE, MARKER = range(8)
 SPLIT_DRIFT_KICK, SPLIT_BEND_KICK, SPLIT_MATRIX_KICK = range(3)
-SPLIT_NAMES = {SPLIT_DRIFT_KICK: "drift_kick", SPLIT_BEND_KICK: "bend_kick", SPLIT_MATRIX_KICK: "matrix_kick"}
+# the same splits with the fourth-order composition of every non-exact slice map (gst.h)
+SPLIT_DRIFT_KICK_4, SPLIT_BEND_KICK_4, SPLIT_MATRIX_KICK_4 = range(3, 6)
+SPLIT_NAMES = {SPLIT_DRIFT_KICK: "drift_kick", SPLIT_BEND_KICK: "bend_kick", SPLIT_MATRIX_KICK: "matrix_kick",
+               SPLIT_DRIFT_KICK_4: "drift_kick_4", SPLIT_BEND_KICK_4: "bend_kick_4", SPLIT_MATRIX_KICK_4: "matrix_kick_4"}
 
 G_PROTON = 1.792847            # BASELINE.json
 MASS_PROTON_EV = 938.27208816e6

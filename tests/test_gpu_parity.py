@@ -291,6 +291,15 @@ def test_config5_sweep_points_reduced(gst, O, split):
         assert np.max(np.abs(pol - rp)) < 1e-6
 
 
+def test_config5_reference_run(gst, O):
+    """The sweep's reference by refinement (matrix-kick, 128 slices, depth 6; studies.py) equals the oracle's."""
+    c = W.config(5, n_particles=24)
+    ref, rlost, _ = O.track(c["lattice"], c["beam"], c["state"], 3, W.SPLIT_MATRIX_KICK, 128, 6)
+    got, lost, pol, emit, _ = gpu_track(gst, c["lattice"], c["beam"], c["state"], 3, W.SPLIT_MATRIX_KICK, 128, 6)
+    assert not rlost.any() and not lost.any()
+    assert orbit_err(got, ref) < 1e-10 and spin_err(got, ref) < 1e-10, (orbit_err(got, ref), spin_err(got, ref))
+
+
 def test_config3_full_size_sampled_particles(gst, O):
     """65536 particles x 1000 turns in the launch configuration bench.py times; the oracle tracks a
     sample of the same particles one by one (particles are independent)."""
