@@ -40,11 +40,18 @@ typedef enum {
   GST_MARKER = 7
 } gst_elem_type;
 
-/* which integrator each thick magnet uses (".apdf"; reading A16) */
+/* which integrator each thick magnet uses (".apdf"; reading A16).  The *_4 values take the
+ * same splits with every second-order slice map (27) replaced by the fourth-order symmetric composition
+ * S2(x1 ds) S2(x0 ds) S2(x1 ds), x1 = 1/(2 - 2^(1/3)), x0 = 1 - 2 x1 ("higher-order versions of
+ * (27)"; reading R5); exact maps (sector bends under bend-/matrix-kick, drifts) are unchanged, and the spin
+ * integrator still samples Omega at the slice edges only.                                              */
 typedef enum {
-  GST_SPLIT_DRIFT_KICK = 0,  /* bends (30)(31), quads and multipoles (29)           */
-  GST_SPLIT_BEND_KICK = 1,   /* bends exact (10), quads and multipoles (29)         */
-  GST_SPLIT_MATRIX_KICK = 2  /* bends exact (10), quads (24)(25)(27): paper's BK/MK */
+  GST_SPLIT_DRIFT_KICK = 0,    /* bends (30)(31), quads and multipoles (29)           */
+  GST_SPLIT_BEND_KICK = 1,     /* bends exact (10), quads and multipoles (29)         */
+  GST_SPLIT_MATRIX_KICK = 2,   /* bends exact (10), quads (24)(25)(27): paper's BK/MK */
+  GST_SPLIT_DRIFT_KICK_4 = 3,
+  GST_SPLIT_BEND_KICK_4 = 4,
+  GST_SPLIT_MATRIX_KICK_4 = 5
 } gst_split;
 
 /* One lattice element.  Plain data, 144 bytes, HOST memory, copied by gst_lattice_create.

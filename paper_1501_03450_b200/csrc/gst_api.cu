@@ -101,25 +101,31 @@ gst::DevElem derive(const gst_element& e, int n_slices, double C) {
     d.ome = (double)((h - k0) / h);
     d.inv_eta = (double)(h / k0);
     d.inv_h = (double)(1.0L / h);
-    long double phi = 0.5L * h * ds;
-    long double q = sinl(0.5L * phi);
-    d.hc = (double)cosl(phi);
-    d.hs = (double)sinl(phi);
-    d.ht = (double)tanl(phi);
-    d.hcm = (double)(2.0L * q * q);
-    d.hsec = (double)(1.0L / cosl(phi));
-    d.r_secm1 = (double)((2.0L * q * q / cosl(phi)) / h);
-    d.r_tan = (double)(tanl(phi) / h);
-    // tan(phi) - phi: series for small phi (long double subtraction would lose digits)
-    long double tmp;
-    if (fabsl(phi) < 0.05L) {
-      long double p2 = phi * phi;
-      tmp = phi * p2 * (1.0L / 3 + p2 * (2.0L / 15 + p2 * (17.0L / 315 + p2 * (62.0L / 2835 + p2 * (1382.0L / 155925 +
-            p2 * (21844.0L / 6081075 + p2 * (929569.0L / 638512875)))))));
-    } else {
-      tmp = tanl(phi) - phi;
+    // TEAPOT curved drifts: ds/2 (second order), x1 ds/2 and (x1 + x0) ds/2 (fourth order, merged neighbours)
+    const long double x1 = 1.0L / (2.0L - cbrtl(2.0L)), x0 = 1.0L - 2.0L * x1;
+    const long double lens[3] = {0.5L * ds, 0.5L * x1 * ds, 0.5L * (x1 + x0) * ds};
+    for (int k = 0; k < 3; ++k) {
+      gst::TeapotHalf& t = d.th[k];
+      long double phi = h * lens[k];
+      long double q = sinl(0.5L * phi);
+      t.len = (double)lens[k];
+      t.c = (double)cosl(phi);
+      t.s = (double)sinl(phi);
+      t.t = (double)tanl(phi);
+      t.sec = (double)(1.0L / cosl(phi));
+      t.r_secm1 = (double)((2.0L * q * q / cosl(phi)) / h);
+      t.r_tan = (double)(tanl(phi) / h);
+      // tan(phi) - phi: series for small phi (long double subtraction would lose digits)
+      long double tmp;
+      if (fabsl(phi) < 0.05L) {
+        long double p2 = phi * phi;
+        tmp = phi * p2 * (1.0L / 3 + p2 * (2.0L / 15 + p2 * (17.0L / 315 + p2 * (62.0L / 2835 + p2 * (1382.0L / 155925 +
+              p2 * (21844.0L / 6081075 + p2 * (929569.0L / 638512875)))))));
+      } else {
+        tmp = tanl(phi) - phi;
+      }
+      t.r_tanmphi = (double)(tmp / h);
     }
-    d.r_tanmphi = (double)(tmp / h);
   }
   if (e.type == GST_RFCAV) {
     d.volt = e.volt_eV;
@@ -177,9 +183,9 @@ SmemPlan plan_smem(size_t tab_bytes, size_t seq_bytes, size_t fixed, size_t budg
   return p;
 }
 
-template <int SPLIT, int DEPTH>
+template <int SPLIT, int DEPTH, int ORDER>
 cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, bool pair, cudaStream_t st) {
-  if (pair) {
+  if (pair && ORDER == 2) {     // the experimental pair kernel exists for the second-order maps only
     // T1p: two threads per particle.  Shared memory per block is budgeted so that MIN_BLOCKS blocks stay
     // resident per SM (227 kB usable, 1 kB reserved per block).
     using Cfg = gst::PairCfg<DEPTH>;
@@ -202,7 +208,7 @@ cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, b
     return cudaGetLastError();
   }
   // T1: one thread per particle; shared memory kept small so that 8 blocks of 64 threads stay resident
-  auto kern = gst::track_kernel<SPLIT, DEPTH>;
+  auto kern = gst::track_kernel<SPLIT, DEPTH, ORDER>;
   SmemPlan p = plan_smem(tab_bytes, seq_bytes, 0, 24 * 1024);
   a.use_smem_seq = p.use_smem_seq;
   if (p.bytes > 48 * 1024) {
@@ -214,21 +220,21 @@ cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, b
   return cudaGetLastError();
 }
 
-template <int SPLIT>
+template <int SPLIT, int ORDER>
 cudaError_t launch_track_depth(int depth, const gst::TrackArgs& a, size_t tb, size_t sb, bool pair, cudaStream_t st) {
   switch (depth) {
-    case 1: return launch_track<SPLIT, 1>(a, tb, sb, pair, st);
-    case 2: return launch_track<SPLIT, 2>(a, tb, sb, pair, st);
-    case 3: return launch_track<SPLIT, 3>(a, tb, sb, pair, st);
-    case 4: return launch_track<SPLIT, 4>(a, tb, sb, pair, st);
-    case 5: return launch_track<SPLIT, 5>(a, tb, sb, pair, st);
-    default: return launch_track<SPLIT, 6>(a, tb, sb, pair, st);
+    case 1: return launch_track<SPLIT, 1, ORDER>(a, tb, sb, pair, st);
+    case 2: return launch_track<SPLIT, 2, ORDER>(a, tb, sb, pair, st);
+    case 3: return launch_track<SPLIT, 3, ORDER>(a, tb, sb, pair, st);
+    case 4: return launch_track<SPLIT, 4, ORDER>(a, tb, sb, pair, st);
+    case 5: return launch_track<SPLIT, 5, ORDER>(a, tb, sb, pair, st);
+    default: return launch_track<SPLIT, 6, ORDER>(a, tb, sb, pair, st);
   }
 }
 
 gst_status validate_track(const gst_lattice* lat, int64_t n_turns, int split, int n_slices, int depth) {
   if (n_turns < 0) return fail(GST_EINVAL, "n_turns < 0");
-  if (split < 0 || split > 2) return fail(GST_EINVAL, "unknown split %d", split);
+  if (split < 0 || split > 5) return fail(GST_EINVAL, "unknown split %d", split);
   if (n_slices < 1 || n_slices > (1 << 20)) return fail(GST_EINVAL, "n_slices must be >= 1");
   if (depth < 1 || depth > 6) return fail(GST_EINVAL, "romberg_depth must be in 1..6");
   for (const gst_element& e : lat->uniq)
@@ -394,9 +400,12 @@ gst_status gst_track(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, gst_
   cudaStream_t st = (cudaStream_t)cuda_stream;
   cudaError_t ce;
   switch (split) {
-    case GST_SPLIT_DRIFT_KICK: ce = launch_track_depth<gst::SPLIT_DK>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
-    case GST_SPLIT_BEND_KICK: ce = launch_track_depth<gst::SPLIT_BK>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
-    default: ce = launch_track_depth<gst::SPLIT_MK>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
+    case GST_SPLIT_DRIFT_KICK: ce = launch_track_depth<gst::SPLIT_DK, 2>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
+    case GST_SPLIT_BEND_KICK: ce = launch_track_depth<gst::SPLIT_BK, 2>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
+    case GST_SPLIT_MATRIX_KICK: ce = launch_track_depth<gst::SPLIT_MK, 2>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
+    case GST_SPLIT_DRIFT_KICK_4: ce = launch_track_depth<gst::SPLIT_DK, 4>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
+    case GST_SPLIT_BEND_KICK_4: ce = launch_track_depth<gst::SPLIT_BK, 4>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
+    default: ce = launch_track_depth<gst::SPLIT_MK, 4>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
   }
   if (ce != cudaSuccess) return fail(GST_ECUDA, "track launch: %s", cudaGetErrorString(ce));
   // host-side bookkeeping of the reference energy: the same IEEE additions the kernel performs

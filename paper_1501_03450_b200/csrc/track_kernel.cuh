@@ -24,6 +24,22 @@ namespace gst {
 enum : int { K_DRIFT = 0, K_SBEND = 1, K_QUAD = 2, K_MULT = 3, K_THIN = 4, K_RF = 5, K_SNAKE = 6, K_MARKER = 7 };
 enum : int { SPLIT_DK = 0, SPLIT_BK = 1, SPLIT_MK = 2 };
 
+// Fourth-order symmetric composition of a second-order slice map S2 (R5):
+//   S4(ds) = S2(x1 ds) S2(x0 ds) S2(x1 ds),  x1 = 1/(2 - 2^(1/3)),  x0 = 1 - 2 x1.
+// Neighbouring exact pieces (half drifts, curved drifts, linear quadrupole flows) are merged by their
+// group property: A(x1/2) B(x1) A((x1+x0)/2) B(x0) A((x1+x0)/2) B(x1) A(x1/2).
+#define GST_YOSHIDA_X1 1.3512071919596576340476878089715
+#define GST_YOSHIDA_X0 (-1.7024143839193152680953756179429)
+
+// constants of one curved drift (31) of length `len` in a bend of curvature h: phi = h len
+struct TeapotHalf {
+  double len;
+  double c, s, t, sec;   // cos phi, sin phi, tan phi, 1/cos phi
+  double r_secm1;        // rho (sec phi - 1)
+  double r_tan;          // rho tan phi
+  double r_tanmphi;      // rho (tan phi - phi)
+};
+
 // Unique-element record, derived on the host for one value of n_slices (a0).
 struct __align__(16) DevElem {
   int type;
@@ -41,13 +57,9 @@ struct __align__(16) DevElem {
   double ome;     // 1 - eta
   double inv_eta; // h/k0
   double inv_h;   // 1/h
-  // sector bend, TEAPOT half drift over ds/2 (phi = h ds/2)
-  double hc, hs, ht;   // cos phi, sin phi, tan phi
-  double hcm;          // 1 - cos phi
-  double r_secm1;      // rho (sec phi - 1)
-  double r_tan;        // rho tan phi
-  double r_tanmphi;    // rho (tan phi - phi)
-  double hsec;         // sec phi
+  // sector bend, TEAPOT curved drifts (31): [0] over ds/2 (second order), [1] over x1 ds/2 and [2] over
+  // (x1 + x0) ds/2 < 0 (the merged neighbours of the fourth-order composition, see Yoshida below)
+  TeapotHalf th[3];
   double kn[4], ks[4]; // multipole strengths (28); thin: integrated
   // cavity
   double volt, krf_over_beta, phi_s, sign, dEs;
@@ -442,11 +454,11 @@ __device__ __forceinline__ bool sbend_exact(State& z, const DevElem& e, const PC
 // a5: TEAPOT sector bend (30)(31): half curved drift, kick -ds k0 (1+hX), half curved drift.
 // The curved drift is a straight line seen from the rotating frame, so (Px,Ps) simply rotate by
 // phi = h ds/2; X, Y, T use rho(sec phi - 1), rho tan phi and rho(tan phi - phi) from the host.
-struct BendTeapot {
+template <int ORDER> struct BendTeapot {
   State& z;
   const DevElem& e;
   const PCon& c;
-  double Ps, iPs, pa2, q2, a1k, hds;
+  double Ps, iPs, pa2, q2, a1k;
   bool bad;
   __device__ __forceinline__ BendTeapot(State& z_, const DevElem& e_, const PCon& c_) : z(z_), e(e_), c(c_) {
     pa2 = fma(-z.Py, z.Py, 1.0 + c.e0);
@@ -456,33 +468,47 @@ struct BendTeapot {
     Ps = ps2 * iPs;
     q2 = c.a2p * e.k0 * z.Py;
     a1k = fma(c.a1, e.k0, -q2 * z.Py);
-    hds = 0.5 * e.ds;
   }
-  __device__ __forceinline__ void half_drift() {
+  // curved drift (31) of length t.len; on entry iPs = 1/Ps
+  __device__ __forceinline__ void curved_drift(const TeapotHalf& t) {
     const double xp = z.Px * iPs;
-    const double D = fma(-xp, e.ht, 1.0);
+    const double D = fma(-xp, t.t, 1.0);
     bad |= !(D > 0.0);
     const double iD = rcp_nr(D);
-    // delta q = [(rho+X) tan phi - s Ps D]/(Ps D),  s = ds/2
-    const double num = e.r_tanmphi + fma(z.X, e.ht, hds * fma(z.Px, e.ht, -(Ps - 1.0)));
+    // delta q = [(rho+X) tan phi - len Ps D]/(Ps D)
+    const double num = t.r_tanmphi + fma(z.X, t.t, t.len * fma(z.Px, t.t, -(Ps - 1.0)));
     const double dq = num * iPs * iD;
-    z.X = (e.r_secm1 + fma(z.X, e.hsec, e.r_tan * xp)) * iD;
-    z.Y = fma(z.Py, hds + dq, z.Y);
-    z.T += fma(-z.Pt, hds, -c.ibpt * dq);
-    const double Pxn = fma(z.Px, e.hc, Ps * e.hs);
-    Ps = fma(Ps, e.hc, -z.Px * e.hs);
+    z.X = (t.r_secm1 + fma(z.X, t.sec, t.r_tan * xp)) * iD;
+    z.Y = fma(z.Py, t.len + dq, z.Y);
+    z.T += fma(-z.Pt, t.len, -c.ibpt * dq);
+    const double Pxn = fma(z.Px, t.c, Ps * t.s);
+    Ps = fma(Ps, t.c, -z.Px * t.s);
     z.Px = Pxn;
     bad |= !(Ps > 0.0);
   }
-  __device__ __forceinline__ void advance() {
-    iPs = rcp_nr(Ps);
-    half_drift();
-    z.Px = fma(-e.ds * e.k0, fma(e.h, z.X, 1.0), z.Px);
+  // kick of (30c) over `len`, then the new longitudinal momentum
+  __device__ __forceinline__ void kick(double len) {
+    z.Px = fma(-len * e.k0, fma(e.h, z.X, 1.0), z.Px);
     const double ps2 = fma(-z.Px, z.Px, pa2);
     bad |= !(ps2 > 0.0);
     iPs = rsqrt_nr(ps2);
     Ps = ps2 * iPs;
-    half_drift();
+  }
+  __device__ __forceinline__ void advance() {
+    iPs = rcp_nr(Ps);
+    if (ORDER == 2) {
+      curved_drift(e.th[0]);
+      kick(e.ds);
+      curved_drift(e.th[0]);
+    } else {
+      curved_drift(e.th[1]);
+      kick(GST_YOSHIDA_X1 * e.ds);
+      curved_drift(e.th[2]);
+      kick(GST_YOSHIDA_X0 * e.ds);
+      curved_drift(e.th[2]);
+      kick(GST_YOSHIDA_X1 * e.ds);
+      curved_drift(e.th[1]);
+    }
   }
   __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) const {
     const double fw = fma(e.h, z.X, 1.0) * rcp_nr(Ps) * w;
@@ -492,9 +518,9 @@ struct BendTeapot {
     ws = fq * Ps;
   }
 };
-template <class Spin>
+template <int ORDER, class Spin>
 __device__ __forceinline__ bool sbend_teapot(State& z, const DevElem& e, const PCon& c, Spin& spin) {
-  BendTeapot s(z, e, c);
+  BendTeapot<ORDER> s(z, e, c);
   spin.run(s, e.N, e.ds);
   return !s.bad;
 }
@@ -525,7 +551,7 @@ __device__ __forceinline__ void omega_straight(double w, double Px, double Py, d
 // a7: drift-kick multipole (29): half drift, kick (28), half drift.  The momenta are constant
 // between kicks, so one 1/Ps serves the second half drift, the edge Omega and the next first half.
 // PURE = quadrupole term only (the common case): field and kick collapse to two FMAs.
-template <bool PURE> struct MultDK {
+template <bool PURE, int ORDER> struct MultDK {
   State& z;
   const DevElem& e;
   const PCon& c;
@@ -550,25 +576,38 @@ template <bool PURE> struct MultDK {
     bad = false;
     momenta();
   }
-  __device__ __forceinline__ void half_drift() {
-    const double l = hds * iPs;
+  __device__ __forceinline__ void drift_by(double len) {
+    const double l = len * iPs;
     z.X = fma(l, z.Px, z.X);
     z.Y = fma(l, z.Py, z.Y);
-    z.T = fma(hds, tnum, z.T);
+    z.T = fma(len, tnum, z.T);
   }
-  __device__ __forceinline__ void advance() {
-    half_drift();
+  __device__ __forceinline__ void kick_by(double len, double lenk) {    // lenk = len * k1
     if (PURE) {
-      z.Px = fma(-dsk, z.X, z.Px);
-      z.Py = fma(dsk, z.Y, z.Py);
+      z.Px = fma(-lenk, z.X, z.Px);
+      z.Py = fma(lenk, z.Y, z.Py);
     } else {
       double bx, by;
       mult_field(e, z.X, z.Y, bx, by);
-      z.Px = fma(-e.ds, by, z.Px);
-      z.Py = fma(e.ds, bx, z.Py);
+      z.Px = fma(-len, by, z.Px);
+      z.Py = fma(len, bx, z.Py);
     }
     momenta();
-    half_drift();
+  }
+  __device__ __forceinline__ void advance() {
+    if (ORDER == 2) {
+      drift_by(hds);
+      kick_by(e.ds, dsk);
+      drift_by(hds);
+    } else {
+      drift_by(GST_YOSHIDA_X1 * hds);
+      kick_by(GST_YOSHIDA_X1 * e.ds, GST_YOSHIDA_X1 * dsk);
+      drift_by((GST_YOSHIDA_X1 + GST_YOSHIDA_X0) * hds);
+      kick_by(GST_YOSHIDA_X0 * e.ds, GST_YOSHIDA_X0 * dsk);
+      drift_by((GST_YOSHIDA_X1 + GST_YOSHIDA_X0) * hds);
+      kick_by(GST_YOSHIDA_X1 * e.ds, GST_YOSHIDA_X1 * dsk);
+      drift_by(GST_YOSHIDA_X1 * hds);
+    }
   }
   __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) const {
     if (PURE) {
@@ -584,14 +623,14 @@ template <bool PURE> struct MultDK {
     }
   }
 };
-template <class Spin>
+template <int ORDER, class Spin>
 __device__ __forceinline__ bool mult_dk(State& z, const DevElem& e, const PCon& c, const Ref& r, Spin& spin) {
   if (e.pure_quad) {
-    MultDK<true> s(z, e, c, r);
+    MultDK<true, ORDER> s(z, e, c, r);
     spin.run(s, e.N, e.ds);
     return !s.bad;
   }
-  MultDK<false> s(z, e, c, r);
+  MultDK<false, ORDER> s(z, e, c, r);
   spin.run(s, e.N, e.ds);
   return !s.bad;
 }
@@ -655,43 +694,61 @@ __device__ __forceinline__ void quadlin_apply(const QuadLin& q, double& uf, doub
   pd = fma(pd, q.Ch, q.kSh * ud);
   ud = nu;
 }
-template <bool FOC> struct QuadMK {
+template <bool FOC, int ORDER> struct QuadMK {
   State& z;
   const PCon& c;
-  QuadLin ql;
+  QuadLin ql;       // linear flow over ds/2 (second order) or x1 ds/2 (fourth order)
+  QuadLin ql2;      // fourth order only: linear flow over (x1 + x0) ds/2 < 0
   double k1, ds, tfac, P2, hiP3, a1k;
   bool bad;
   __device__ __forceinline__ QuadMK(State& z_, const DevElem& e, const PCon& c_) : z(z_), c(c_) {
     k1 = e.kn[0];
     ds = e.ds;
-    quadlin_build(ql, fabs(k1), 0.5 * e.ds, c);
+    if (ORDER == 2) {
+      quadlin_build(ql, fabs(k1), 0.5 * e.ds, c);
+    } else {
+      quadlin_build(ql, fabs(k1), (0.5 * GST_YOSHIDA_X1) * e.ds, c);
+      quadlin_build(ql2, fabs(k1), (0.5 * (GST_YOSHIDA_X1 + GST_YOSHIDA_X0)) * e.ds, c);
+    }
     tfac = c.iP * c.ibpt;
     P2 = 1.0 + c.e0;
     hiP3 = 0.5 * c.iP * c.iP * c.iP;
     a1k = c.a1 * k1;
     bad = false;
   }
-  __device__ __forceinline__ void lin() {
-    if (FOC) quadlin_apply(ql, z.X, z.Px, z.Y, z.Py, z.T, tfac);
-    else     quadlin_apply(ql, z.Y, z.Py, z.X, z.Px, z.T, tfac);
+  __device__ __forceinline__ void lin(const QuadLin& q) {
+    if (FOC) quadlin_apply(q, z.X, z.Px, z.Y, z.Py, z.T, tfac);
+    else     quadlin_apply(q, z.Y, z.Py, z.X, z.Px, z.T, tfac);
+  }
+  // (25) over `len`: X += len Px (1/Ps - 1/P), 1/Ps - 1/P = pt2/(P Ps (P+Ps))
+  __device__ __forceinline__ void nonlinear(double len) {
+    const double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
+    const double ps2 = P2 - pt2;
+    bad |= !(ps2 > 0.0);
+    const double iPs = rsqrt_nr(ps2);
+    const double Ps = ps2 * iPs;
+    const double t = iPs * rcp_nr(c.P + Ps);         // 1/(Ps (P+Ps))
+    const double d = pt2 * c.iP * t;
+    z.X = fma(len * d, z.Px, z.X);
+    z.Y = fma(len * d, z.Py, z.Y);
+    // T' = -(1/beta0+Pt)[1/Ps - 1/P - pt2/(2P^3)] + tq,  bracket = pt2^2 (2P+Ps)/(2 P^3 Ps (P+Ps)^2)
+    const double br = pt2 * pt2 * fma(2.0, c.P, Ps) * hiP3 * t * (t * Ps);
+    z.T = fma(len, fma(-c.ibpt, br, c.tq), z.T);
   }
   __device__ __forceinline__ void advance() {
-    lin();
-    {   // (25): X += ds Px (1/Ps - 1/P), 1/Ps - 1/P = pt2/(P Ps (P+Ps))
-      const double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
-      const double ps2 = P2 - pt2;
-      bad |= !(ps2 > 0.0);
-      const double iPs = rsqrt_nr(ps2);
-      const double Ps = ps2 * iPs;
-      const double t = iPs * rcp_nr(c.P + Ps);         // 1/(Ps (P+Ps))
-      const double d = pt2 * c.iP * t;
-      z.X = fma(ds * d, z.Px, z.X);
-      z.Y = fma(ds * d, z.Py, z.Y);
-      // T' = -(1/beta0+Pt)[1/Ps - 1/P - pt2/(2P^3)] + tq,  bracket = pt2^2 (2P+Ps)/(2 P^3 Ps (P+Ps)^2)
-      const double br = pt2 * pt2 * fma(2.0, c.P, Ps) * hiP3 * t * (t * Ps);
-      z.T = fma(ds, fma(-c.ibpt, br, c.tq), z.T);
+    if (ORDER == 2) {
+      lin(ql);
+      nonlinear(ds);
+      lin(ql);
+    } else {
+      lin(ql);
+      nonlinear(GST_YOSHIDA_X1 * ds);
+      lin(ql2);
+      nonlinear(GST_YOSHIDA_X0 * ds);
+      lin(ql2);
+      nonlinear(GST_YOSHIDA_X1 * ds);
+      lin(ql);
     }
-    lin();
   }
   __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) {
     const double ps2 = P2 - fma(z.Px, z.Px, z.Py * z.Py);
@@ -704,14 +761,14 @@ template <bool FOC> struct QuadMK {
     ws = w * pb;
   }
 };
-template <class Spin>
+template <int ORDER, class Spin>
 __device__ __forceinline__ bool quad_mk(State& z, const DevElem& e, const PCon& c, Spin& spin) {
   if (e.kn[0] > 0.0) {
-    QuadMK<true> s(z, e, c);
+    QuadMK<true, ORDER> s(z, e, c);
     spin.run(s, e.N, e.ds);
     return !s.bad;
   }
-  QuadMK<false> s(z, e, c);
+  QuadMK<false, ORDER> s(z, e, c);
   spin.run(s, e.N, e.ds);
   return !s.bad;
 }
@@ -720,15 +777,15 @@ __device__ __forceinline__ bool quad_mk(State& z, const DevElem& e, const PCon& 
 // one element (the dispatch is uniform across the grid: every particle is in the same element)
 // ---------------------------------------------------------------------------------------------
 // The tests are ordered by how often each type occurs in a ring (drifts, quadrupoles, bends, thin lenses).
-template <int SPLIT, class Spin>
+template <int SPLIT, int ORDER, class Spin>
 __device__ __forceinline__ bool element_step(int type, State& z, const DevElem& e, PCon& pc, Ref& ref, double G, Spin& spin) {
   if (type == K_DRIFT) return drift(z, e.L, pc, ref);
   if (type == K_QUAD) {
-    if (SPLIT == SPLIT_MK) return quad_mk(z, e, pc, spin);
-    return mult_dk(z, e, pc, ref, spin);
+    if (SPLIT == SPLIT_MK) return quad_mk<ORDER>(z, e, pc, spin);
+    return mult_dk<ORDER>(z, e, pc, ref, spin);
   }
   if (type == K_SBEND) {
-    if (SPLIT == SPLIT_DK) return sbend_teapot(z, e, pc, spin);
+    if (SPLIT == SPLIT_DK) return sbend_teapot<ORDER>(z, e, pc, spin);
     return sbend_exact(z, e, pc, ref, spin);
   }
   if (type == K_THIN) {   // A10: half kick, spin, half kick
@@ -744,7 +801,7 @@ __device__ __forceinline__ bool element_step(int type, State& z, const DevElem& 
     z.Py = fma(0.5, bx, z.Py);
     return ok;
   }
-  if (type == K_MULT) return mult_dk(z, e, pc, ref, spin);
+  if (type == K_MULT) return mult_dk<ORDER>(z, e, pc, ref, spin);
   if (type == K_RF) {     // A12, A13
     double krf = e.krf_over_beta * ref.beta0;
     double dE = e.volt * sin(fma(e.sign * krf, z.T, e.phi_s));
@@ -775,7 +832,7 @@ __device__ __forceinline__ bool element_step(int type, State& z, const DevElem& 
 constexpr int TRACK_BLOCK = 64;
 constexpr int TRACK_MIN_BLOCKS = 8;
 
-template <int SPLIT, int DEPTH>
+template <int SPLIT, int DEPTH, int ORDER>
 __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_kernel(const TrackArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   DevElem* tab = reinterpret_cast<DevElem*>(smem_raw);
@@ -814,7 +871,7 @@ __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_kernel(co
       const uint32_t cur = nxt;
       nxt = seq[ie + 1 < a.n_seq ? ie + 1 : 0];          // next element's entry, one element ahead
       const DevElem& e = tab[cur >> 8];
-      const bool ok = element_step<SPLIT>((int)(cur & 0xffu), z, e, pc, ref, a.G, spin);
+      const bool ok = element_step<SPLIT, ORDER>((int)(cur & 0xffu), z, e, pc, ref, a.G, spin);
       if (!ok) {
         lost = true;
         z.X = z.Px = z.Y = z.Py = z.T = z.Pt = 0.0;

@@ -159,7 +159,7 @@ __device__ __forceinline__ void orbit_role(const TrackArgs& a, const DevElem* ta
     for (int ie = 0; ie < a.n_seq; ++ie) {
       const uint32_t cur = seq[ie];
       const DevElem& e = tab[cur >> 8];
-      const bool ok = element_step<SPLIT>((int)(cur & 0xffu), z, e, pc, ref, a.G, spin);
+      const bool ok = element_step<SPLIT, 2>((int)(cur & 0xffu), z, e, pc, ref, a.G, spin);
       if (!ok) {
         // A15: the particle is lost.  The warp must stay in step with its partner, so the lane goes on
         // with the reference orbit (all zeros); nothing of it is stored.

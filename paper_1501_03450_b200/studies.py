@@ -104,11 +104,15 @@ def sweep(args):
         b.close()
         return dev, ms, int(lost)
 
-    ref, ref_ms, ref_lost = run(W.SPLIT_MATRIX_KICK, args.ref_slices, 6)
-    print(json.dumps(dict(study="sweep", reference=dict(split="matrix_kick", n_slices=args.ref_slices, depth=6, ms=ref_ms,
+    ref_split = W.SPLIT_MATRIX_KICK_4 if args.order4 else W.SPLIT_MATRIX_KICK
+    ref, ref_ms, ref_lost = run(ref_split, args.ref_slices, 6)
+    print(json.dumps(dict(study="sweep", reference=dict(split=W.SPLIT_NAMES[ref_split], n_slices=args.ref_slices, depth=6, ms=ref_ms,
                                                         lost=ref_lost), particles=n, turns=turns)))
     rows = []
-    for split in (W.SPLIT_DRIFT_KICK, W.SPLIT_BEND_KICK, W.SPLIT_MATRIX_KICK):
+    splits = [W.SPLIT_DRIFT_KICK, W.SPLIT_BEND_KICK, W.SPLIT_MATRIX_KICK]
+    if args.order4:
+        splits += [W.SPLIT_DRIFT_KICK_4, W.SPLIT_BEND_KICK_4, W.SPLIT_MATRIX_KICK_4]
+    for split in splits:
         for n_slices, depth in W.sweep_pairs():
             if n_slices > args.max_slices:
                 continue
@@ -126,9 +130,10 @@ def sweep(args):
     if args.out:
         with open(args.out, "w") as f:
             f.write("# Accuracy vs throughput (config 5): RHIC-like ring without snakes, %d particles, %d turns\n\n" % (n, turns))
-            f.write("Command: `python -m paper_1501_03450_b200.studies sweep --particles %d --turns %d`\n\n" % (n, turns))
-            f.write("Reference: matrix-kick, %d slices, depth 6 (%.1f s).  spin error = (46) P:733, X error = (44) P:622.\n\n"
-                    % (args.ref_slices, ref_ms * 1e-3))
+            f.write("Command: `python -m paper_1501_03450_b200.studies sweep --particles %d --turns %d%s`\n\n"
+                    % (n, turns, " --order4" if args.order4 else ""))
+            f.write("Reference: %s, %d slices, depth 6 (%.1f s).  spin error = (46) P:733, X error = (44) P:622.\n\n"
+                    % (W.SPLIT_NAMES[ref_split], args.ref_slices, ref_ms * 1e-3))
             f.write("| split | slices | depth | spin error | rms X error [m] | steps/s | particle-turns/s |\n|---|---|---|---|---|---|---|\n")
             for r in rows:
                 f.write("| %s | %d | %d | %.3e | %.3e | %.4g | %.4g |\n" % (r["split"], r["n_slices"], r["depth"], r["spin_err"],
@@ -149,6 +154,8 @@ def main(argv=None):
     s.add_argument("--turns", type=int, default=None)
     s.add_argument("--ref-slices", type=int, default=128)
     s.add_argument("--max-slices", type=int, default=64)
+    s.add_argument("--order4", action="store_true",
+                   help="add the fourth-order compositions (SURVEY 8(f) f1); the reference becomes matrix_kick_4")
     s.add_argument("--out", default=None)
     args = ap.parse_args(argv)
     t0 = time.time()
