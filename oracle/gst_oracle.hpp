@@ -409,6 +409,50 @@ template <class R> bool orbit_slice(Orbit<R>& z, const Element& e, R ds, int spl
   return orbit_slice2(z, e, x1 * ds, base, ref);
 }
 
+// Piece-wise constant spin precession (37) P:470-482 with Omega taken in the MIDDLE of each slice; the two
+// orderings the paper names in the caption of Fig. 14:
+//   PWC_HALF_SLICE (depth  0)  "DKDSDKD": half a slice map, spin rotation R(ds Omega), half a slice map --
+//                              for any split (the half map is the split's own second-/fourth-order map over ds/2)
+//   PWC_DKSKD      (depth -1)  "DKSKD": half drift, half kick, spin rotation, half kick, half drift -- for the
+//                              elements integrated by a drift-kick map (29) or (30)(31); others as PWC_HALF_SLICE
+// The spin is rotated slice by slice, later rotations on the left (37b).  DESIGN.md reading R7.
+enum { PWC_HALF_SLICE = 0, PWC_DKSKD = -1 };
+
+template <class R> bool track_thick_pwc(Particle<R>& p, const Element& e, const Reference<R>& ref, double G,
+                                        int split, int N, R ds, int kind) {
+  const int base = split % 3;
+  const bool drift_kick_map = (e.type == SBEND) ? (base == SPLIT_DRIFT_KICK)
+                                                : !(e.type == QUAD && base == SPLIT_MATRIX_KICK);
+  for (int i = 0; i < N; ++i) {
+    Vec3<R> Om;
+    if (kind == PWC_DKSKD && drift_kick_map) {
+      const R h2 = ds / R(2);
+      if (e.type == SBEND) {
+        if (!curved_drift(p.z, h2, R(e.h), ref)) return false;
+        bend_kick(p.z, h2, R(e.h), R(e.k0));
+      } else {
+        if (!drift(p.z, h2, ref)) return false;
+        multipole_kick(p.z, h2, e.kn, e.ks);
+      }
+      if (!omega_tbmt(p.z, R(e.h), element_field(e, p.z), G, ref, Om)) return false;
+      p.S = quat_rotate(quat_from_rotvec(Vec3<R>{ds * Om.x, ds * Om.y, ds * Om.s}), p.S);
+      if (e.type == SBEND) {
+        bend_kick(p.z, h2, R(e.h), R(e.k0));
+        if (!curved_drift(p.z, h2, R(e.h), ref)) return false;
+      } else {
+        multipole_kick(p.z, h2, e.kn, e.ks);
+        if (!drift(p.z, h2, ref)) return false;
+      }
+    } else {
+      if (!orbit_slice(p.z, e, ds / R(2), split, ref)) return false;
+      if (!omega_tbmt(p.z, R(e.h), element_field(e, p.z), G, ref, Om)) return false;
+      p.S = quat_rotate(quat_from_rotvec(Vec3<R>{ds * Om.x, ds * Om.y, ds * Om.s}), p.S);
+      if (!orbit_slice(p.z, e, ds / R(2), split, ref)) return false;
+    }
+  }
+  return true;
+}
+
 // returns false if the particle is lost inside this element (A15): p is then restored to its
 // value at the element entrance.
 template <class R> bool track_element(Particle<R>& p, const Element& e, Reference<R>& ref, double G,
@@ -421,6 +465,10 @@ template <class R> bool track_element(Particle<R>& p, const Element& e, Referenc
     case SBEND: case QUAD: case MULTIPOLE: {
       int N = n_slices * e.slice_mult;
       R ds = R(e.L) / R(N);
+      if (depth <= 0) {                                              // comparison integrators of section 4.1
+        ok = track_thick_pwc(p, e, ref, G, split, N, ds, depth);
+        break;
+      }
       std::vector<Vec3<R>> Om(N + 1);
       ok = omega_tbmt(p.z, R(e.h), element_field(e, p.z), G, ref, Om[0]);
       for (int i = 1; ok && i <= N; ++i) {

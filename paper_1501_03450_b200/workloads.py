@@ -19,6 +19,8 @@ DRIFT, SBEND, QUAD, MULTIPOLE, THINMULT, RFCAV, SNAKE, MARKER = range(8)
 SPLIT_DRIFT_KICK, SPLIT_BEND_KICK, SPLIT_MATRIX_KICK = range(3)
 # the same splits with the fourth-order composition of every non-exact slice map (gst.h)
 SPLIT_DRIFT_KICK_4, SPLIT_BEND_KICK_4, SPLIT_MATRIX_KICK_4 = range(3, 6)
+# spin ordering of the mid-slice piece-wise-constant comparison integrators ((37); gst_track_pwc)
+PWC_HALF_SLICE, PWC_DKSKD = 0, -1
 SPLIT_NAMES = {SPLIT_DRIFT_KICK: "drift_kick", SPLIT_BEND_KICK: "bend_kick", SPLIT_MATRIX_KICK: "matrix_kick",
                SPLIT_DRIFT_KICK_4: "drift_kick_4", SPLIT_BEND_KICK_4: "bend_kick_4", SPLIT_MATRIX_KICK_4: "matrix_kick_4"}
 
