@@ -110,6 +110,17 @@ void gst_bunch_destroy(gst_bunch* b);
 gst_status gst_track(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, gst_split split, int n_slices,
                      int romberg_depth, void* cuda_stream);
 
+/* The comparison integrators of the paper's section 4.1 (Figs. 7, 14): the same orbit maps, but the
+ * spin is rotated once per slice by R(ds Omega) with Omega taken in the MIDDLE of the slice (37), no Romberg.
+ *   GST_PWC_HALF_SLICE  half a slice map, spin rotation, half a slice map ("DKDSDKD"); any split
+ *   GST_PWC_DKSKD       half drift, half kick, spin rotation, half kick, half drift ("DKSKD") in the
+ *                       elements a drift-kick map integrates under `split`; the others as GST_PWC_HALF_SLICE
+ * Second-order splits only (GST_EINVAL for GST_SPLIT_*_4).  Otherwise exactly like gst_track: asynchronous,
+ * in place, one launch.                                                                              */
+typedef enum { GST_PWC_HALF_SLICE = 0, GST_PWC_DKSKD = 1 } gst_pwc_order;
+gst_status gst_track_pwc(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, gst_split split, int n_slices,
+                         gst_pwc_order order, void* cuda_stream);
+
 /* Which tracking kernel gst_track launches (process-wide; results are bit-identical):
  *   GST_KERNEL_FUSED  one thread per particle, orbit and spin work software-pipelined -- default
  *   GST_KERNEL_PAIR   experimental: an orbit thread and a spin thread per particle, coupled through a

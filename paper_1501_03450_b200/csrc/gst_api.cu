@@ -103,8 +103,8 @@ gst::DevElem derive(const gst_element& e, int n_slices, double C) {
     d.inv_h = (double)(1.0L / h);
     // TEAPOT curved drifts: ds/2 (second order), x1 ds/2 and (x1 + x0) ds/2 (fourth order, merged neighbours)
     const long double x1 = 1.0L / (2.0L - cbrtl(2.0L)), x0 = 1.0L - 2.0L * x1;
-    const long double lens[3] = {0.5L * ds, 0.5L * x1 * ds, 0.5L * (x1 + x0) * ds};
-    for (int k = 0; k < 3; ++k) {
+    const long double lens[4] = {0.5L * ds, 0.5L * x1 * ds, 0.5L * (x1 + x0) * ds, ds};
+    for (int k = 0; k < 4; ++k) {
       gst::TeapotHalf& t = d.th[k];
       long double phi = h * lens[k];
       long double q = sinl(0.5L * phi);
@@ -185,7 +185,8 @@ SmemPlan plan_smem(size_t tab_bytes, size_t seq_bytes, size_t fixed, size_t budg
 
 template <int SPLIT, int DEPTH, int ORDER>
 cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, bool pair, cudaStream_t st) {
-  if (pair && ORDER == 2) {     // the experimental pair kernel exists for the second-order maps only
+  if constexpr (ORDER == 2 && DEPTH >= 1) {   // the experimental pair kernel: second-order maps, edge scheme only
+  if (pair) {
     // T1p: two threads per particle.  Shared memory per block is budgeted so that MIN_BLOCKS blocks stay
     // resident per SM (227 kB usable, 1 kB reserved per block).
     using Cfg = gst::PairCfg<DEPTH>;
@@ -207,6 +208,7 @@ cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, b
     kern<<<blocks, Cfg::THREADS, p.bytes, st>>>(a);
     return cudaGetLastError();
   }
+  }
   // T1: one thread per particle; shared memory kept small so that 8 blocks of 64 threads stay resident
   auto kern = gst::track_kernel<SPLIT, DEPTH, ORDER>;
   SmemPlan p = plan_smem(tab_bytes, seq_bytes, 0, 24 * 1024);
@@ -222,6 +224,8 @@ cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, b
 
 template <int SPLIT, int ORDER>
 cudaError_t launch_track_depth(int depth, const gst::TrackArgs& a, size_t tb, size_t sb, bool pair, cudaStream_t st) {
+  if (ORDER == 2 && depth == 0) return launch_track<SPLIT, 0, 2>(a, tb, sb, false, st);
+  if (ORDER == 2 && depth == -1) return launch_track<SPLIT, -1, 2>(a, tb, sb, false, st);
   switch (depth) {
     case 1: return launch_track<SPLIT, 1, ORDER>(a, tb, sb, pair, st);
     case 2: return launch_track<SPLIT, 2, ORDER>(a, tb, sb, pair, st);
@@ -366,11 +370,16 @@ gst_status gst_bunch_set_reference(gst_bunch* b, const gst_beam* beam, int64_t t
   return GST_OK;
 }
 
-gst_status gst_track(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, gst_split split, int n_slices,
-                     int romberg_depth, void* cuda_stream) {
+// depth_code >= 1: trapezoid/Romberg scheme of that depth; 0 / -1: mid-slice PWC (half-slice / DKSKD ordering),
+// for which the element table is derived for 2 n_slices half slices
+static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, gst_split split, int n_slices,
+                             int depth_code, void* cuda_stream) {
   if (!b || !lat) return fail(GST_EINVAL, "null handle");
-  gst_status vs = validate_track(lat, n_turns, (int)split, n_slices, romberg_depth);
+  gst_status vs = validate_track(lat, n_turns, (int)split, n_slices, depth_code >= 1 ? depth_code : 1);
   if (vs != GST_OK) return vs;
+  if (depth_code < 1 && (int)split > 2) return fail(GST_EINVAL, "gst_track_pwc takes the second-order splits only");
+  const int romberg_depth = depth_code;
+  const int table_slices = depth_code >= 1 ? n_slices : 2 * n_slices;
   if (!b->have_ref) {
     b->E0 = lat->beam.gamma0 * lat->beam.mass_eV;
     b->mass = lat->beam.mass_eV;
@@ -378,7 +387,7 @@ gst_status gst_track(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, gst_
   }
   if (b->n == 0 || n_turns == 0) return GST_OK;
   const gst::DevElem* d_tab = nullptr;
-  gst_status ts = get_table(lat, n_slices, &d_tab);
+  gst_status ts = get_table(lat, table_slices, &d_tab);
   if (ts != GST_OK) return ts;
   gst::TrackArgs a;
   for (int i = 0; i < 9; ++i) a.p[i] = b->p[i];
@@ -414,6 +423,18 @@ gst_status gst_track(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, gst_
       if (dEs != 0.0) b->E0 = b->E0 + dEs;
   b->turn += n_turns;
   return GST_OK;
+}
+
+gst_status gst_track(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, gst_split split, int n_slices,
+                     int romberg_depth, void* cuda_stream) {
+  if (romberg_depth < 1) return fail(GST_EINVAL, "romberg_depth must be in 1..6");
+  return track_impl(b, lat, n_turns, split, n_slices, romberg_depth, cuda_stream);
+}
+
+gst_status gst_track_pwc(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, gst_split split, int n_slices,
+                         gst_pwc_order order, void* cuda_stream) {
+  if (order != GST_PWC_HALF_SLICE && order != GST_PWC_DKSKD) return fail(GST_EINVAL, "unknown PWC ordering %d", (int)order);
+  return track_impl(b, lat, n_turns, split, n_slices, order == GST_PWC_HALF_SLICE ? 0 : -1, cuda_stream);
 }
 
 static gst_status run_moments(gst_bunch* b, cudaStream_t st, bool second) {

@@ -58,8 +58,9 @@ struct __align__(16) DevElem {
   double inv_eta; // h/k0
   double inv_h;   // 1/h
   // sector bend, TEAPOT curved drifts (31): [0] over ds/2 (second order), [1] over x1 ds/2 and [2] over
-  // (x1 + x0) ds/2 < 0 (the merged neighbours of the fourth-order composition, see Yoshida below)
-  TeapotHalf th[3];
+  // (x1 + x0) ds/2 < 0 (the merged neighbours of the fourth-order composition, see Yoshida above), [3] over ds
+  // (the whole drifts of the DKSKD ordering, whose table is derived for half slices)
+  TeapotHalf th[4];
   double kn[4], ks[4]; // multipole strengths (28); thin: integrated
   // cavity
   double volt, krf_over_beta, phi_s, sign, dEs;
@@ -376,6 +377,42 @@ template <int DEPTH> struct FusedSpin {
   __device__ __forceinline__ void snake(const Quat& q) { quat_rotate(q, Sx, Sy, Ss); }
 };
 
+// Mid-slice piece-wise-constant precession (37) P:470-482, the comparison integrator of Figs. 7 and 14.
+// KIND = 0: half slice map, rotation by ds*Omega(mid), half slice map ("DKDSDKD"); KIND = -1: half drift,
+// half kick, rotation, half kick, half drift ("DKSKD") in drift-kick-mapped elements.  The element table is
+// derived for HALF slices: N2 = 2 N maps of length ds2 = ds/2, one rotation of weight 2 ds2 per pair.
+template <int KIND> struct MidSpin {
+  double &Sx, &Sy, &Ss;
+  __device__ __forceinline__ MidSpin(State& z) : Sx(z.Sx), Sy(z.Sy), Ss(z.Ss) {}
+  template <class Stepper>
+  __device__ __forceinline__ void run(Stepper& s, int N2, double ds2) {
+    constexpr bool DKSKD = KIND == -1;
+    const double w = 2.0 * ds2;
+    double wx, wy, ws;
+    s.template pwc_first<DKSKD>();
+    s.omega(w, wx, wy, ws);
+    Quat Q = quat_from_rotvec(wx, wy, ws);
+    s.template pwc_second<DKSKD>();
+    for (int i = 2; i < N2; i += 2) {
+      s.template pwc_first<DKSKD>();
+      s.omega(w, wx, wy, ws);
+      Q = quat_mul(quat_from_rotvec(wx, wy, ws), Q);        // later rotations on the left (37b)
+      s.template pwc_second<DKSKD>();
+    }
+    const double rn = rsqrt_nr(fma(Q.w, Q.w, fma(Q.x, Q.x, fma(Q.y, Q.y, Q.s * Q.s))));
+    Q.w *= rn; Q.x *= rn; Q.y *= rn; Q.s *= rn;
+    quat_rotate(Q, Sx, Sy, Ss);
+  }
+  __device__ __forceinline__ void thin(double wx, double wy, double ws) {
+    Quat q = quat_from_rotvec(wx, wy, ws);
+    quat_rotate(q, Sx, Sy, Ss);
+  }
+  __device__ __forceinline__ void snake(const Quat& q) { quat_rotate(q, Sx, Sy, Ss); }
+};
+template <int DEPTH> struct SpinPolicy { using type = FusedSpin<DEPTH>; };
+template <> struct SpinPolicy<0> { using type = MidSpin<0>; };
+template <> struct SpinPolicy<-1> { using type = MidSpin<-1>; };
+
 // a4: exact sector bend (10), spin from the slice-edge Omega (6b).
 // With c = cos(h ds), s = sin(h ds), A = sqrt(Pa^2 - Px^2), g = A - eta(1 + hX):
 //   Px_f = Px + [g s - Px (1-c)]                                                    (10b)
@@ -413,6 +450,8 @@ struct BendExact {
     Am1 = fma(-dPx, rr, Am1);
     Px = Pxf; A = Af; iA = y;
   }
+  template <bool DKSKD> __device__ __forceinline__ void pwc_first() { advance(); }     // exact map: half slice
+  template <bool DKSKD> __device__ __forceinline__ void pwc_second() { advance(); }
   // Omega = -(1+hX)/Ps [a1 b - a2 (u.b) u] + h y-hat with b = (0, k0, 0), Ps = A
   __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) const {
     const double fw = fma(h, X, 1.0) * iA * w;
@@ -509,6 +548,13 @@ template <int ORDER> struct BendTeapot {
       kick(GST_YOSHIDA_X1 * e.ds);
       curved_drift(e.th[1]);
     }
+  }
+  // mid-slice PWC (37): the element table is derived for HALF slices (e.ds = half the spin slice)
+  template <bool DKSKD> __device__ __forceinline__ void pwc_first() {
+    if (DKSKD) { iPs = rcp_nr(Ps); curved_drift(e.th[3]); kick(e.ds); } else advance();
+  }
+  template <bool DKSKD> __device__ __forceinline__ void pwc_second() {
+    if (DKSKD) { kick(e.ds); curved_drift(e.th[3]); } else advance();
   }
   __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) const {
     const double fw = fma(e.h, z.X, 1.0) * rcp_nr(Ps) * w;
@@ -608,6 +654,12 @@ template <bool PURE, int ORDER> struct MultDK {
       kick_by(GST_YOSHIDA_X1 * e.ds, GST_YOSHIDA_X1 * dsk);
       drift_by(GST_YOSHIDA_X1 * hds);
     }
+  }
+  template <bool DKSKD> __device__ __forceinline__ void pwc_first() {
+    if (DKSKD) { drift_by(e.ds); kick_by(e.ds, dsk); } else advance();
+  }
+  template <bool DKSKD> __device__ __forceinline__ void pwc_second() {
+    if (DKSKD) { kick_by(e.ds, dsk); drift_by(e.ds); } else advance();
   }
   __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) const {
     if (PURE) {
@@ -750,6 +802,8 @@ template <bool FOC, int ORDER> struct QuadMK {
       lin(ql);
     }
   }
+  template <bool DKSKD> __device__ __forceinline__ void pwc_first() { advance(); }     // not a drift-kick map: half slice
+  template <bool DKSKD> __device__ __forceinline__ void pwc_second() { advance(); }
   __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) {
     const double ps2 = P2 - fma(z.Px, z.Px, z.Py * z.Py);
     bad |= !(ps2 > 0.0);
@@ -863,7 +917,7 @@ __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_kernel(co
   // loads and the type dispatch are warp-uniform (uniform registers, no divergence bookkeeping); a
   // particle that is lost (A15) goes on with the reference orbit and nothing of it is stored.
   bool lost = false;
-  FusedSpin<DEPTH> spin(z);
+  typename SpinPolicy<DEPTH>::type spin(z);
   uint32_t nxt = seq[0];
   for (long long turn = 0; turn < a.n_turns; ++turn) {
 #pragma unroll 1

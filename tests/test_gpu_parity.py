@@ -36,11 +36,15 @@ def O():
 
 
 def gpu_track(gst, lat, beam, state, n_turns, split, n_slices, depth, chunks=None):
+    """depth >= 1: gst_track; depth = W.PWC_HALF_SLICE / W.PWC_DKSKD (0 / -1): gst_track_pwc"""
     L = gst.Lattice(lat, beam)
     d = torch.tensor(state, dtype=torch.float64, device="cuda").contiguous()
     b = gst.Bunch(d)
     for nt in (chunks or [n_turns]):
-        b.track(L, nt, split, n_slices, depth)
+        if depth >= 1:
+            b.track(L, nt, split, n_slices, depth)
+        else:
+            b.track_pwc(L, nt, split, n_slices, depth)
     pol, nlost = b.polarization()
     emit = b.emittance()
     lost = b.lost()
@@ -141,6 +145,33 @@ def test_order4_config3_ring_and_accuracy_gain(gst, O, split):
     e4 = np.sqrt(np.mean((got[0] - fine[0]) ** 2))
     e2 = np.sqrt(np.mean((second[0] - fine[0]) ** 2))
     assert e4 < 0.2 * e2, (e4, e2)
+
+
+@pytest.mark.parametrize("split", [W.SPLIT_DRIFT_KICK, W.SPLIT_BEND_KICK, W.SPLIT_MATRIX_KICK])
+@pytest.mark.parametrize("order", [W.PWC_HALF_SLICE, W.PWC_DKSKD])
+@pytest.mark.parametrize("n_slices", [1, 3, 8])
+def test_pwc_mid_slice_integrators_all_element_types(gst, O, split, order, n_slices):
+    """gst_track_pwc (section 4.1, (37)) against the oracle, every element type."""
+    lat = mixed_lattice()
+    bm = W.beam(12.0)
+    st = W.gaussian_bunch(13, 200, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
+    ref, rlost, g_ref = O.track(lat, bm, st, 2, split, n_slices, order)
+    got, lost, pol, emit, g_gpu = gpu_track(gst, lat, bm, st, 2, split, n_slices, order)
+    assert not rlost.any() and not lost.any()
+    assert orbit_err(got, ref) < 2e-12, orbit_err(got, ref)
+    assert spin_err(got, ref) < 2e-12, spin_err(got, ref)
+    assert abs(g_gpu - g_ref) < 1e-12 * g_ref
+
+
+def test_pwc_rejects_fourth_order_splits(gst):
+    c = W.config(1)
+    L = gst.Lattice(c["lattice"], c["beam"])
+    b = gst.Bunch(torch.tensor(c["state"], dtype=torch.float64, device="cuda"))
+    with pytest.raises(gst.GstError) as ei:
+        b.track_pwc(L, 1, W.SPLIT_BEND_KICK_4, 4, W.PWC_HALF_SLICE)
+    assert ei.value.status == gst.EINVAL
+    b.close()
+    L.close()
 
 
 def test_large_angle_per_slice_takes_the_sincos_branch(gst, O):
