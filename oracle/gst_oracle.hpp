@@ -33,7 +33,8 @@ namespace orc {
 // ----------------------------------------------------------------------------------------------
 // element table entry (the oracle's own definition; field meaning identical to DESIGN.md §2)
 // ----------------------------------------------------------------------------------------------
-enum ElemType { DRIFT = 0, SBEND = 1, QUAD = 2, MULTIPOLE = 3, THINMULT = 4, RFCAV = 5, SNAKE = 6, MARKER = 7 };
+enum ElemType { DRIFT = 0, SBEND = 1, QUAD = 2, MULTIPOLE = 3, THINMULT = 4, RFCAV = 5, SNAKE = 6, MARKER = 7,
+                FRINGE = 8 };   // thin-fringe spin kick (41) P:557-563, SURVEY 8(f) f3
 enum Split { SPLIT_DRIFT_KICK = 0, SPLIT_BEND_KICK = 1, SPLIT_MATRIX_KICK = 2,
              // the same splits with every second-order slice map (27) replaced by the fourth-order symmetric
              // composition of three of them ("more sophisticated symmetric compositions", "higher-order
@@ -461,6 +462,22 @@ template <class R> bool track_element(Particle<R>& p, const Element& e, Referenc
   bool ok = true;
   switch (e.type) {
     case MARKER: break;
+    case FRINGE: {
+      // (41) P:561: thin fringe of a 2m-pole, lowest order: rotation about s-hat by
+      //   omega = -(+-)(1+G) [b_m r^m sin(m phi) + a_m r^m cos(m phi)]/(m (B rho)_o),  (X+iY)^m = r^m e^(i m phi),
+      // + on entering (e.sign = +1), - on leaving (e.sign = -1).  m = 1 is the dipole term b_1 = k0;
+      // kn[m-2], ks[m-2] hold m = 2..5 in the convention of (28).  The orbit is not touched (reading R8).
+      R re = p.z.X, im = p.z.Y;                                      // (X + iY)^m, m = 1
+      R psi = R(e.k0) * im;
+      for (int m = 2; m <= 5; ++m) {
+        R nre = re * p.z.X - im * p.z.Y, nim = re * p.z.Y + im * p.z.X;
+        re = nre; im = nim;
+        psi = psi + (R(e.kn[m - 2]) * im + R(e.ks[m - 2]) * re) / R(m);
+      }
+      R om = -R(e.sign) * R(1.0 + G) * psi;
+      p.S = quat_rotate(quat_from_rotvec(Vec3<R>{R(0), R(0), om}), p.S);
+      break;
+    }
     case DRIFT: ok = drift(p.z, R(e.L), ref); break;                 // one exact step, no field, no spin (A17)
     case SBEND: case QUAD: case MULTIPOLE: {
       int N = n_slices * e.slice_mult;

@@ -15,7 +15,7 @@ import math
 
 import numpy as np
 
-DRIFT, SBEND, QUAD, MULTIPOLE, THINMULT, RFCAV, SNAKE, MARKER = range(8)
+DRIFT, SBEND, QUAD, MULTIPOLE, THINMULT, RFCAV, SNAKE, MARKER, FRINGE = range(9)
 SPLIT_DRIFT_KICK, SPLIT_BEND_KICK, SPLIT_MATRIX_KICK = range(3)
 # the same splits with the fourth-order composition of every non-exact slice map (gst.h)
 SPLIT_DRIFT_KICK_4, SPLIT_BEND_KICK_4, SPLIT_MATRIX_KICK_4 = range(3, 6)
@@ -97,6 +97,24 @@ def snake(mu, phi):
 
 def marker():
     return _blank(MARKER)
+
+
+def fringe(sign, k0=0.0, kn=(0, 0, 0, 0), ks=(0, 0, 0, 0)):
+    """Thin-fringe spin kick (41) of a magnet with body strengths k0 (dipole), kn, ks (m = 2..5, per unit length,
+    convention of (28)); sign = +1 at the entrance, -1 at the exit."""
+    e = _blank(FRINGE)
+    e["k0"] = k0
+    e["kn"] = kn
+    e["ks"] = ks
+    e["sign"] = sign
+    return e
+
+
+def with_fringes(magnet):
+    """[entrance fringe, magnet, exit fringe] for a thick SBEND / QUAD / MULTIPOLE element."""
+    k0 = float(magnet["k0"]) if int(magnet["type"]) == SBEND else 0.0
+    kn, ks = tuple(magnet["kn"]), tuple(magnet["ks"])
+    return [fringe(+1.0, k0, kn, ks), magnet, fringe(-1.0, k0, kn, ks)]
 
 
 def lattice(elems):
