@@ -37,7 +37,11 @@ typedef enum {
   GST_THINMULT = 4,  /* thin lens, "drift-kick without the drift" P:378                             */
   GST_RFCAV = 5,     /* thin RF cavity with optional reference-energy ramp                          */
   GST_SNAKE = 6,     /* Siberian snake: orbit-transparent thin spin rotation P:585                  */
-  GST_MARKER = 7
+  GST_MARKER = 7,
+  GST_FRINGE = 8     /* thin-fringe spin kick (41) P:561 of a magnet with body strengths k0 (dipole, m = 1), kn, ks
+                        (m = 2..5, per unit length): rotation about s-hat by
+                        -sign (1+G) [k0 Y + sum_m (kn Im (X+iY)^m + ks Re (X+iY)^m)/m]; sign = +1 at the
+                        entrance, -1 at the exit; orbit-transparent (the paper gives no orbital fringe map)  */
 } gst_elem_type;
 
 /* which integrator each thick magnet uses (".apdf"; reading A16).  The *_4 values take the
@@ -68,7 +72,8 @@ typedef struct {
   double volt_eV;     /* RFCAV: q*V peak energy gain [eV]                                         */
   double harmonic;    /* RFCAV: harmonic number; k_rf = 2 pi harmonic beta_o / C, C = sum of L    */
   double phi_s;       /* RFCAV: synchronous phase [rad]; reference energy += volt_eV*sin(phi_s)   */
-  double sign;        /* RFCAV: +1/-1, dE = volt_eV*sin(phi_s + sign*k_rf*T)  (+1 above transition) */
+  double sign;        /* RFCAV: +1/-1, dE = volt_eV*sin(phi_s + sign*k_rf*T)  (+1 above transition);
+                         FRINGE: +1 entrance, -1 exit                                             */
   double snake_mu;    /* SNAKE: rotation angle [rad]                                              */
   double snake_phi;   /* SNAKE: axis (sin phi, 0, cos phi) in (x,y,s): angle from s-hat in the x-s plane */
 } gst_element;

@@ -134,6 +134,7 @@ gst::DevElem derive(const gst_element& e, int n_slices, double C) {
     d.sign = e.sign;
     d.dEs = e.volt_eV * std::sin(e.phi_s);
   }
+  if (e.type == GST_FRINGE) d.sign = e.sign;
   if (e.type == GST_SNAKE) {
     double sh = std::sin(0.5 * e.snake_mu);
     d.qw = std::cos(0.5 * e.snake_mu);
@@ -267,7 +268,7 @@ gst_status gst_lattice_create(const gst_element* elems, size_t n, const gst_beam
   if (!(beam->gamma0 > 1.0) || !(beam->mass_eV > 0.0)) return fail(GST_EINVAL, "beam: need gamma0 > 1 and mass_eV > 0");
   for (size_t i = 0; i < n; ++i) {
     const gst_element& e = elems[i];
-    if (e.type < 0 || e.type > GST_MARKER) return fail(GST_EINVAL, "element %zu: unknown type %d", i, e.type);
+    if (e.type < 0 || e.type > GST_FRINGE) return fail(GST_EINVAL, "element %zu: unknown type %d", i, e.type);
     if ((is_thick(e.type) || e.type == GST_DRIFT) && !(e.L > 0.0)) return fail(GST_EINVAL, "element %zu: L must be > 0", i);
     if (is_thick(e.type) && e.slice_mult < 1) return fail(GST_EINVAL, "element %zu: slice_mult must be >= 1", i);
     if (e.type == GST_SBEND && (e.h == 0.0 || e.k0 == 0.0)) return fail(GST_EINVAL, "element %zu: SBEND needs h != 0 and k0 != 0", i);

@@ -21,7 +21,7 @@
 
 namespace gst {
 
-enum : int { K_DRIFT = 0, K_SBEND = 1, K_QUAD = 2, K_MULT = 3, K_THIN = 4, K_RF = 5, K_SNAKE = 6, K_MARKER = 7 };
+enum : int { K_DRIFT = 0, K_SBEND = 1, K_QUAD = 2, K_MULT = 3, K_THIN = 4, K_RF = 5, K_SNAKE = 6, K_MARKER = 7, K_FRINGE = 8 };
 enum : int { SPLIT_DK = 0, SPLIT_BK = 1, SPLIT_MK = 2 };
 
 // Fourth-order symmetric composition of a second-order slice map S2 (R5):
@@ -830,6 +830,8 @@ __device__ __forceinline__ bool quad_mk(State& z, const DevElem& e, const PCon& 
 // ---------------------------------------------------------------------------------------------
 // one element (the dispatch is uniform across the grid: every particle is in the same element)
 // ---------------------------------------------------------------------------------------------
+__constant__ double FRINGE_INV_M[4] = {1.0 / 2.0, 1.0 / 3.0, 1.0 / 4.0, 1.0 / 5.0};
+
 // The tests are ordered by how often each type occurs in a ring (drifts, quadrupoles, bends, thin lenses).
 template <int SPLIT, int ORDER, class Spin>
 __device__ __forceinline__ bool element_step(int type, State& z, const DevElem& e, PCon& pc, Ref& ref, double G, Spin& spin) {
@@ -872,6 +874,17 @@ __device__ __forceinline__ bool element_step(int type, State& z, const DevElem& 
     return true;
   }
   if (type == K_SNAKE) spin.snake(Quat{e.qw, e.qx, e.qy, e.qs});
+  if (type == K_FRINGE) {   // thin-fringe spin kick (41) P:561: rotation about s-hat, orbit untouched
+    double re = z.X, im = z.Y;                       // (X + iY)^m
+    double psi = e.k0 * im;                          // m = 1
+    const int top = e.order;
+    for (int m = 2; m <= top; ++m) {
+      const double nre = fma(re, z.X, -im * z.Y), nim = fma(re, z.Y, im * z.X);
+      re = nre; im = nim;
+      psi = fma(fma(e.kn[m - 2], im, e.ks[m - 2] * re), FRINGE_INV_M[m - 2], psi);
+    }
+    spin.thin(0.0, 0.0, -e.sign * (1.0 + G) * psi);  // e.sign = +1 entering, -1 leaving
+  }
   return true;
 }
 

@@ -174,6 +174,28 @@ def test_pwc_rejects_fourth_order_splits(gst):
     L.close()
 
 
+@pytest.mark.parametrize("variant", ["fused", "pair"])
+def test_thin_fringe_spin_kicks(gst, O, variant):
+    """GST_FRINGE (41) P:561 around every thick magnet of the mixed lattice."""
+    els = []
+    for e in mixed_lattice():
+        els += W.with_fringes(e) if int(e["type"]) in (W.SBEND, W.QUAD, W.MULTIPOLE) else [e]
+    lat = W.lattice(els)
+    bm = W.beam(12.0)
+    st = W.gaussian_bunch(17, 200, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
+    ref, rlost, _ = O.track(lat, bm, st, 2, W.SPLIT_MATRIX_KICK, 4, 3)
+    plain, _, _ = O.track(mixed_lattice(), bm, st, 2, W.SPLIT_MATRIX_KICK, 4, 3)
+    try:
+        gst.set_kernel_variant(gst.KERNEL_PAIR if variant == "pair" else gst.KERNEL_FUSED)
+        got, lost, pol, emit, _ = gpu_track(gst, lat, bm, st, 2, W.SPLIT_MATRIX_KICK, 4, 3)
+    finally:
+        gst.set_kernel_variant(gst.KERNEL_FUSED)
+    assert not rlost.any() and not lost.any()
+    assert orbit_err(got, ref) < 2e-12 and spin_err(got, ref) < 2e-12, (orbit_err(got, ref), spin_err(got, ref))
+    assert spin_err(plain, ref) > 1e-6                       # the kicks are not a no-op on this bunch
+    assert np.array_equal(plain[:6], ref[:6])                # and leave the orbit alone
+
+
 def test_large_angle_per_slice_takes_the_sincos_branch(gst, O):
     # one slice through a strong bend at high G*gamma: rotation angle per edge > 1.4 rad
     lat = W.lattice([W.sbend(9.45, 0.2), W.drift(1.0)])
