@@ -34,7 +34,8 @@ namespace orc {
 // element table entry (the oracle's own definition; field meaning identical to DESIGN.md §2)
 // ----------------------------------------------------------------------------------------------
 enum ElemType { DRIFT = 0, SBEND = 1, QUAD = 2, MULTIPOLE = 3, THINMULT = 4, RFCAV = 5, SNAKE = 6, MARKER = 7,
-                FRINGE = 8 };   // thin-fringe spin kick (41) P:557-563, SURVEY 8(f) f3
+                FRINGE = 8,     // thin-fringe spin kick (41) P:557-563, SURVEY 8(f) f3
+                SOLENOID = 9 }; // solenoid with thin-pancake fringes (32)-(36), (40) P:420-464, f4
 enum Split { SPLIT_DRIFT_KICK = 0, SPLIT_BEND_KICK = 1, SPLIT_MATRIX_KICK = 2,
              // the same splits with every second-order slice map (27) replaced by the fourth-order symmetric
              // composition of three of them ("more sophisticated symmetric compositions", "higher-order
@@ -370,6 +371,48 @@ template <class R> Vec3<R> element_field(const Element& e, const Orbit<R>& z) {
   return Vec3<R>{bx, by, R(0)};
 }
 
+// ---- solenoid (section 3.7).  e.k0 holds b_0/(B rho)_o, so eta = e.k0/2 (35); (e/p_o) A = eta (-Y, X) (32) ----
+// kinetic transverse momenta (36): canonical minus `frac` times the vector potential
+template <class R> Orbit<R> solenoid_kinetic(const Orbit<R>& z, R eta, R frac) {
+  Orbit<R> k = z;
+  k.Px = z.Px + frac * eta * z.Y;
+  k.Py = z.Py - frac * eta * z.X;
+  return k;
+}
+// exact flow of H_sol (33) over s: z <- R2 R1 z on (X, Px, Y, Py), T by (34c); kappa = eta / Ps^i
+template <class R> bool solenoid_body(Orbit<R>& z, R s, R eta, const Reference<R>& ref) {
+  R ps2 = Ps2(solenoid_kinetic(z, eta, R(1)), ref);                  // the square root of (33)
+  if (ps2 <= R(0)) return false;
+  R Ps = m::sqrt(ps2);
+  R kap = eta / Ps;
+  R c = m::cos(kap * s), sn = m::sin(kap * s);
+  R X1 = c * z.X + sn / eta * z.Px, Px1 = -eta * sn * z.X + c * z.Px;   // (34a)
+  R Y1 = c * z.Y + sn / eta * z.Py, Py1 = -eta * sn * z.Y + c * z.Py;
+  z.X = c * X1 + sn * Y1;    z.Px = c * Px1 + sn * Py1;                 // (34b)
+  z.Y = -sn * X1 + c * Y1;   z.Py = -sn * Px1 + c * Py1;
+  z.T = z.T - (R(1) / ref.beta0 + z.Pt) * s / Ps + s / ref.beta0;       // (34c)
+  return true;
+}
+// Omega (6b) in the body: B/(B rho)_o = (0, 0, 2 eta), u-hat from the KINETIC momentum (36)
+template <class R> bool solenoid_omega(const Orbit<R>& z, R eta, double G, const Reference<R>& ref, Vec3<R>& Om) {
+  return omega_tbmt(solenoid_kinetic(z, eta, R(1)), R(0), Vec3<R>{R(0), R(0), R(2) * eta}, G, ref, Om);
+}
+// thin-pancake fringe spin kick (40) P:553: sign = +1 entrance, -1 exit; kinetic momentum and Ps with A/2
+template <class R> bool solenoid_fringe_rotvec(const Orbit<R>& z, R eta, R sign, double G, const Reference<R>& ref, Vec3<R>& w) {
+  Orbit<R> k = solenoid_kinetic(z, eta, R(1) / R(2));
+  R ps2 = Ps2(k, ref);
+  if (ps2 <= R(0)) return false;
+  R Ps = m::sqrt(ps2), P2 = Ptot2(z, ref);
+  R gamma = ref.gamma0 * (R(1) + ref.beta0 * z.Pt);
+  R a1 = R(1) + R(G) * gamma, a2 = R(G) * (gamma - R(1));
+  R proj = (z.X * k.Px + z.Y * k.Py) / P2;
+  R pre = sign * eta / Ps;
+  w.x = pre * (a1 * z.X - a2 * proj * k.Px);
+  w.y = pre * (a1 * z.Y - a2 * proj * k.Py);
+  w.s = pre * (-a2 * proj * Ps);
+  return true;
+}
+
 // one second-order orbital slice of a thick magnet of the given type with the given split (A16)
 template <class R> bool orbit_slice2(Orbit<R>& z, const Element& e, R ds, int split, const Reference<R>& ref) {
   if (e.type == SBEND) {
@@ -493,6 +536,33 @@ template <class R> bool track_element(Particle<R>& p, const Element& e, Referenc
         if (ok) ok = omega_tbmt(p.z, R(e.h), element_field(e, p.z), G, ref, Om[i]);
       }
       if (ok) p.S = quat_rotate(romberg_quaternion(Om, N, ds, depth), p.S);
+      break;
+    }
+    case SOLENOID: {   // entrance fringe kick (40), body (34) in N exact slices with the edge scheme (38)(39), exit kick
+      const R eta = R(e.k0) / R(2);
+      int N = n_slices * e.slice_mult;
+      R ds = R(e.L) / R(N);
+      Vec3<R> w;
+      ok = solenoid_fringe_rotvec(p.z, eta, R(1), G, ref, w);                 // entrance: +
+      if (!ok) break;
+      p.S = quat_rotate(quat_from_rotvec(w), p.S);
+      if (depth <= 0) {                                              // mid-slice PWC (37): half map, rotation, half map
+        for (int i = 0; ok && i < N; ++i) {
+          Vec3<R> Om;
+          ok = solenoid_body(p.z, ds / R(2), eta, ref) && solenoid_omega(p.z, eta, G, ref, Om);
+          if (!ok) break;
+          p.S = quat_rotate(quat_from_rotvec(Vec3<R>{ds * Om.x, ds * Om.y, ds * Om.s}), p.S);
+          ok = solenoid_body(p.z, ds / R(2), eta, ref);
+        }
+      } else {
+        std::vector<Vec3<R>> Om(N + 1);
+        ok = solenoid_omega(p.z, eta, G, ref, Om[0]);
+        for (int i = 1; ok && i <= N; ++i) ok = solenoid_body(p.z, ds, eta, ref) && solenoid_omega(p.z, eta, G, ref, Om[i]);
+        if (ok) p.S = quat_rotate(romberg_quaternion(Om, N, ds, depth), p.S);
+      }
+      if (!ok) break;
+      ok = solenoid_fringe_rotvec(p.z, eta, R(-1), G, ref, w);                // exit: -
+      if (ok) p.S = quat_rotate(quat_from_rotvec(w), p.S);
       break;
     }
     case THINMULT: {                                                 // A10: half kick, spin, half kick

@@ -15,7 +15,7 @@ import math
 
 import numpy as np
 
-DRIFT, SBEND, QUAD, MULTIPOLE, THINMULT, RFCAV, SNAKE, MARKER, FRINGE = range(9)
+DRIFT, SBEND, QUAD, MULTIPOLE, THINMULT, RFCAV, SNAKE, MARKER, FRINGE, SOLENOID = range(10)
 SPLIT_DRIFT_KICK, SPLIT_BEND_KICK, SPLIT_MATRIX_KICK = range(3)
 # the same splits with the fourth-order composition of every non-exact slice map (gst.h)
 SPLIT_DRIFT_KICK_4, SPLIT_BEND_KICK_4, SPLIT_MATRIX_KICK_4 = range(3, 6)
@@ -110,6 +110,15 @@ def fringe(sign, k0=0.0, kn=(0, 0, 0, 0), ks=(0, 0, 0, 0)):
     return e
 
 
+def solenoid(L, ks, slice_mult=1):
+    """Solenoid with thin-pancake fringes (section 3.7): ks = b_0/(B rho)_o [1/m] (eta of (35) is ks/2)."""
+    e = _blank(SOLENOID)
+    e["L"] = L
+    e["k0"] = ks
+    e["slice_mult"] = slice_mult
+    return e
+
+
 def with_fringes(magnet):
     """[entrance fringe, magnet, exit fringe] for a thick SBEND / QUAD / MULTIPOLE element."""
     k0 = float(magnet["k0"]) if int(magnet["type"]) == SBEND else 0.0
@@ -131,7 +140,7 @@ def beta_of_gamma(g):
 
 def steps_per_turn(lat, n_slices):
     """particle-element-steps per particle per turn."""
-    thick = np.isin(lat["type"], (SBEND, QUAD, MULTIPOLE))
+    thick = np.isin(lat["type"], (SBEND, QUAD, MULTIPOLE, SOLENOID))
     return int(np.sum(np.where(thick, n_slices * lat["slice_mult"], 1)))
 
 
