@@ -38,10 +38,14 @@ typedef enum {
   GST_RFCAV = 5,     /* thin RF cavity with optional reference-energy ramp                          */
   GST_SNAKE = 6,     /* Siberian snake: orbit-transparent thin spin rotation P:585                  */
   GST_MARKER = 7,
-  GST_FRINGE = 8     /* thin-fringe spin kick (41) P:561 of a magnet with body strengths k0 (dipole, m = 1), kn, ks
+  GST_FRINGE = 8,    /* thin-fringe spin kick (41) P:561 of a magnet with body strengths k0 (dipole, m = 1), kn, ks
                         (m = 2..5, per unit length): rotation about s-hat by
                         -sign (1+G) [k0 Y + sum_m (kn Im (X+iY)^m + ks Re (X+iY)^m)/m]; sign = +1 at the
                         entrance, -1 at the exit; orbit-transparent (the paper gives no orbital fringe map)  */
+  GST_SOLENOID = 9   /* solenoid with thin-pancake fringes, section 3.7: k0 = b_0/(B rho)_o [1/m] (eta of (35)
+                        is k0/2), L > 0; exact body flow (34) in n_slices*slice_mult slices for the spin scheme, Omega
+                        with u-hat from the kinetic momentum (36), fringe spin kicks (40) at both ends; the orbit is
+                        canonical throughout (the fringes leave the canonical momenta unchanged)             */
 } gst_elem_type;
 
 /* which integrator each thick magnet uses (".apdf"; reading A16).  The *_4 values take the

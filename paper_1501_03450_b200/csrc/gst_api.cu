@@ -39,7 +39,7 @@ gst_status fail(gst_status s, const char* fmt, ...) {
     if (e_ != cudaSuccess) return fail(GST_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
   } while (0)
 
-bool is_thick(int t) { return t == GST_SBEND || t == GST_QUAD || t == GST_MULTIPOLE; }
+bool is_thick(int t) { return t == GST_SBEND || t == GST_QUAD || t == GST_MULTIPOLE || t == GST_SOLENOID; }
 
 struct DevTable {
   gst::DevElem* d_tab = nullptr;
@@ -268,10 +268,11 @@ gst_status gst_lattice_create(const gst_element* elems, size_t n, const gst_beam
   if (!(beam->gamma0 > 1.0) || !(beam->mass_eV > 0.0)) return fail(GST_EINVAL, "beam: need gamma0 > 1 and mass_eV > 0");
   for (size_t i = 0; i < n; ++i) {
     const gst_element& e = elems[i];
-    if (e.type < 0 || e.type > GST_FRINGE) return fail(GST_EINVAL, "element %zu: unknown type %d", i, e.type);
+    if (e.type < 0 || e.type > GST_SOLENOID) return fail(GST_EINVAL, "element %zu: unknown type %d", i, e.type);
     if ((is_thick(e.type) || e.type == GST_DRIFT) && !(e.L > 0.0)) return fail(GST_EINVAL, "element %zu: L must be > 0", i);
     if (is_thick(e.type) && e.slice_mult < 1) return fail(GST_EINVAL, "element %zu: slice_mult must be >= 1", i);
     if (e.type == GST_SBEND && (e.h == 0.0 || e.k0 == 0.0)) return fail(GST_EINVAL, "element %zu: SBEND needs h != 0 and k0 != 0", i);
+    if (e.type == GST_SOLENOID && e.k0 == 0.0) return fail(GST_EINVAL, "element %zu: SOLENOID needs k0 != 0", i);
     if (e.type == GST_QUAD) {
       if (e.kn[0] == 0.0) return fail(GST_EINVAL, "element %zu: QUAD needs kn[0] != 0", i);
       for (int k = 0; k < 4; ++k)

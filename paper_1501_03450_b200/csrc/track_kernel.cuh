@@ -21,7 +21,7 @@
 
 namespace gst {
 
-enum : int { K_DRIFT = 0, K_SBEND = 1, K_QUAD = 2, K_MULT = 3, K_THIN = 4, K_RF = 5, K_SNAKE = 6, K_MARKER = 7, K_FRINGE = 8 };
+enum : int { K_DRIFT = 0, K_SBEND = 1, K_QUAD = 2, K_MULT = 3, K_THIN = 4, K_RF = 5, K_SNAKE = 6, K_MARKER = 7, K_FRINGE = 8, K_SOLENOID = 9 };
 enum : int { SPLIT_DK = 0, SPLIT_BK = 1, SPLIT_MK = 2 };
 
 // Fourth-order symmetric composition of a second-order slice map S2 (R5):
@@ -830,6 +830,75 @@ __device__ __forceinline__ bool quad_mk(State& z, const DevElem& e, const PCon& 
 // ---------------------------------------------------------------------------------------------
 // one element (the dispatch is uniform across the grid: every particle is in the same element)
 // ---------------------------------------------------------------------------------------------
+// f4: solenoid with thin-pancake fringes (section 3.7).  e.k0 = b_0/(B rho)_o, eta = k0/2 (35).
+// The body flow (34) is exact, so a slice is the same map over ds; Ps of (33) is an invariant of it, which
+// makes kappa = eta/Ps and cos/sin(kappa ds) per-particle constants of the element, and lets T (34c) be
+// applied once (cancellation-free as in drift()).  Omega (6b) takes u-hat from the kinetic momentum (36).
+struct Solenoid {
+  State& z;
+  const PCon& c;
+  double eta, cs, sn, sn_eta, eta_sn, iPs, Ps, two_eta;
+  bool bad;
+  __device__ __forceinline__ Solenoid(State& z_, const DevElem& e, const PCon& c_) : z(z_), c(c_) {
+    eta = 0.5 * e.k0;
+    two_eta = e.k0;
+    const double kx = fma(eta, z.Y, z.Px), ky = fma(-eta, z.X, z.Py);
+    const double ps2 = 1.0 + c.e0 - fma(kx, kx, ky * ky);
+    bad = !(ps2 > 0.0);
+    iPs = rsqrt_nr(bad ? 1.0 : ps2);
+    Ps = ps2 * iPs;
+    sincos(eta * iPs * e.ds, &sn, &cs);
+    sn_eta = sn / eta;
+    eta_sn = eta * sn;
+  }
+  __device__ __forceinline__ void advance() {      // R2 R1 of (34a)(34b)
+    const double X1 = fma(cs, z.X, sn_eta * z.Px), P1 = fma(cs, z.Px, -eta_sn * z.X);
+    const double Y1 = fma(cs, z.Y, sn_eta * z.Py), Q1 = fma(cs, z.Py, -eta_sn * z.Y);
+    z.X = fma(cs, X1, sn * Y1);   z.Px = fma(cs, P1, sn * Q1);
+    z.Y = fma(cs, Y1, -sn * X1);  z.Py = fma(cs, Q1, -sn * P1);
+  }
+  template <bool DKSKD> __device__ __forceinline__ void pwc_first() { advance(); }
+  template <bool DKSKD> __device__ __forceinline__ void pwc_second() { advance(); }
+  // w Omega, b = (0, 0, 2 eta):  (2 eta a2' kx, 2 eta a2' ky, 2 eta (a2' Ps - a1/Ps)),  a2' = G(gamma-1)/P^2
+  __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) const {
+    const double kx = fma(eta, z.Y, z.Px), ky = fma(-eta, z.X, z.Py);
+    const double f = w * two_eta * c.a2p;
+    wx = f * kx;
+    wy = f * ky;
+    ws = fma(f, Ps, -w * two_eta * c.a1 * iPs);
+  }
+  // thin-pancake fringe spin kick (40) P:553: sign = +1 entrance, -1 exit; kinetic momentum and Ps with A/2
+  __device__ __forceinline__ void fringe(double sign, double& wx, double& wy, double& ws) {
+    const double kx = fma(0.5 * eta, z.Y, z.Px), ky = fma(-0.5 * eta, z.X, z.Py);
+    const double ps2 = 1.0 + c.e0 - fma(kx, kx, ky * ky);
+    bad |= !(ps2 > 0.0);
+    const double ips = rsqrt_nr(ps2);
+    const double proj = c.a2p * fma(z.X, kx, z.Y * ky);       // G(gamma-1)(X kx + Y ky)/P^2
+    const double pre = sign * eta * ips;
+    wx = pre * fma(c.a1, z.X, -proj * kx);
+    wy = pre * fma(c.a1, z.Y, -proj * ky);
+    ws = -sign * eta * proj;                                   // pre * (-proj * Ps')
+  }
+};
+template <class Spin>
+__device__ __forceinline__ bool solenoid(State& z, const DevElem& e, const PCon& c, const Ref& r, Spin& spin) {
+  Solenoid s(z, e, c);
+  double wx, wy, ws;
+  s.fringe(+1.0, wx, wy, ws);
+  spin.thin(wx, wy, ws);
+  spin.run(s, e.N, e.ds);
+  s.fringe(-1.0, wx, wy, ws);
+  spin.thin(wx, wy, ws);
+  // (34c) over the whole length, with the kinetic transverse momentum (an invariant of the body flow)
+  const double kx = fma(s.eta, z.Y, z.Px), ky = fma(-s.eta, z.X, z.Py);
+  const double pt2 = fma(kx, kx, ky * ky);
+  const double ps2m1 = c.e0 - pt2;
+  const double iPs1 = rcp_nr(s.Ps + 1.0);
+  const double num = (fma(-pt2, r.ibeta0, c.tA) - z.Pt * ps2m1 * iPs1) * iPs1;
+  z.T = fma(e.L * s.iPs, num, z.T);
+  return !s.bad;
+}
+
 __constant__ double FRINGE_INV_M[4] = {1.0 / 2.0, 1.0 / 3.0, 1.0 / 4.0, 1.0 / 5.0};
 
 // The tests are ordered by how often each type occurs in a ring (drifts, quadrupoles, bends, thin lenses).
@@ -874,6 +943,7 @@ __device__ __forceinline__ bool element_step(int type, State& z, const DevElem& 
     return true;
   }
   if (type == K_SNAKE) spin.snake(Quat{e.qw, e.qx, e.qy, e.qs});
+  if (type == K_SOLENOID) return solenoid(z, e, pc, ref, spin);
   if (type == K_FRINGE) {   // thin-fringe spin kick (41) P:561: rotation about s-hat, orbit untouched
     double re = z.X, im = z.Y;                       // (X + iY)^m
     double psi = e.k0 * im;                          // m = 1

@@ -195,6 +195,12 @@ __device__ __forceinline__ void spin_role(const TrackArgs& a, const DevElem* tab
       const int type = (int)(cur & 0xffu);
       if (type == K_SBEND || type == K_QUAD || type == K_MULT) {
         spin.template thick<DEPTH>(e.N, Sx, Sy, Ss);
+      } else if (type == K_SOLENOID) {            // entrance kick, body, exit kick
+        Quat q = spin.pop();
+        quat_rotate(q, Sx, Sy, Ss);
+        spin.template thick<DEPTH>(e.N, Sx, Sy, Ss);
+        q = spin.pop();
+        quat_rotate(q, Sx, Sy, Ss);
       } else if (type == K_THIN || type == K_FRINGE) {
         Quat q = spin.pop();
         quat_rotate(q, Sx, Sy, Ss);

@@ -196,6 +196,26 @@ def test_thin_fringe_spin_kicks(gst, O, variant):
     assert np.array_equal(plain[:6], ref[:6])                # and leave the orbit alone
 
 
+@pytest.mark.parametrize("variant,depth,n_slices", [("fused", 1, 3), ("fused", 4, 8), ("fused", 6, 32), ("pair", 3, 4),
+                                                    ("fused", W.PWC_HALF_SLICE, 4), ("fused", W.PWC_DKSKD, 4)])
+def test_solenoids_in_a_ring(gst, O, variant, depth, n_slices):
+    """GST_SOLENOID: body (34), kinetic momentum in Omega (36), fringe kicks (40)."""
+    els = list(mixed_lattice())
+    els.insert(3, W.solenoid(2.1, 0.2))                      # the paper's 1.3 T x 2.1 m magnet at a few GeV (P:719)
+    els.insert(20, W.solenoid(0.8, -0.35, slice_mult=2))
+    lat = W.lattice(els)
+    bm = W.beam(3.0)
+    st = W.gaussian_bunch(19, 200, 3.0, 3e-3, 5e-4, 3e-3, 5e-4, 5e-4, 0.05, "sphere")
+    ref, rlost, _ = O.track(lat, bm, st, 2, W.SPLIT_BEND_KICK, n_slices, depth)
+    try:
+        gst.set_kernel_variant(gst.KERNEL_PAIR if variant == "pair" else gst.KERNEL_FUSED)
+        got, lost, pol, emit, _ = gpu_track(gst, lat, bm, st, 2, W.SPLIT_BEND_KICK, n_slices, depth)
+    finally:
+        gst.set_kernel_variant(gst.KERNEL_FUSED)
+    assert not rlost.any() and not lost.any()
+    assert orbit_err(got, ref) < 2e-12 and spin_err(got, ref) < 2e-12, (orbit_err(got, ref), spin_err(got, ref))
+
+
 def test_large_angle_per_slice_takes_the_sincos_branch(gst, O):
     # one slice through a strong bend at high G*gamma: rotation angle per edge > 1.4 rad
     lat = W.lattice([W.sbend(9.45, 0.2), W.drift(1.0)])
