@@ -35,7 +35,8 @@ namespace orc {
 // ----------------------------------------------------------------------------------------------
 enum ElemType { DRIFT = 0, SBEND = 1, QUAD = 2, MULTIPOLE = 3, THINMULT = 4, RFCAV = 5, SNAKE = 6, MARKER = 7,
                 FRINGE = 8,     // thin-fringe spin kick (41) P:557-563, SURVEY 8(f) f3
-                SOLENOID = 9 }; // solenoid with thin-pancake fringes (32)-(36), (40) P:420-464, f4
+                SOLENOID = 9,   // solenoid with thin-pancake fringes (32)-(36), (40) P:420-464, f4
+                RBEND = 10 };   // rectangular bend (11)-(19) P:161-261 with the fringe spin kick (42) P:567, f3
 enum Split { SPLIT_DRIFT_KICK = 0, SPLIT_BEND_KICK = 1, SPLIT_MATRIX_KICK = 2,
              // the same splits with every second-order slice map (27) replaced by the fourth-order symmetric
              // composition of three of them ("more sophisticated symmetric compositions", "higher-order
@@ -371,6 +372,67 @@ template <class R> Vec3<R> element_field(const Element& e, const Orbit<R>& z) {
   return Vec3<R>{bx, by, R(0)};
 }
 
+// ---- rectangular bend (section 3.2).  e.k0 = b_1/(B rho)_o = 1/rho_b (12); e.kn[0], e.kn[1] = phi_entr, phi_exit ----
+// body (13) P:170-186 over the length s along the magnet axis; coordinates internal to the magnet (Cartesian)
+template <class R> bool rbend_body(Orbit<R>& z, R s, R k0, const Reference<R>& ref) {
+  R Pa2 = R(1) + R(2) * z.Pt / ref.beta0 + z.Pt * z.Pt - z.Py * z.Py;             // (8)
+  if (Pa2 <= R(0)) return false;
+  R Pa = m::sqrt(Pa2);
+  R Pxf = z.Px - s * k0;                                                          // (13b)
+  R a2 = Pa2 - z.Px * z.Px, f2 = Pa2 - Pxf * Pxf;
+  if (a2 <= R(0) || f2 <= R(0)) return false;
+  R dasin = m::asin(z.Px / Pa) - m::asin(Pxf / Pa);
+  z.X = z.X + (m::sqrt(f2) - m::sqrt(a2)) / k0;                                   // (13a)
+  z.Y = z.Y + z.Py * dasin / k0;                                                  // (13c)
+  z.T = z.T - (R(1) / ref.beta0 + z.Pt) * dasin / k0;                             // (13e): no +s/beta_o, see (19)
+  z.Px = Pxf;
+  return true;
+}
+// thin-fringe orbit map (15) P:204-224, sign = +1 entrance, -1 exit; "P_c" of (15e) read as P_s (A1)
+template <class R> bool rbend_fringe(Orbit<R>& z, R sign, R k0, const Reference<R>& ref) {
+  R ps2 = Ps2(z, ref);
+  if (ps2 <= R(0)) return false;
+  R Ps = m::sqrt(ps2);
+  R xp = z.Px / Ps, yp = z.Py / Ps, b = sign * k0;
+  R d = R(1) + yp * yp;
+  R arg = R(1) + b * xp * yp / d * R(2) * z.Y;
+  if (arg <= R(0)) return false;
+  R Yf = R(2) * z.Y / (R(1) + m::sqrt(arg));                                      // (15c)
+  z.X = z.X + b / (R(2) * Ps) * ((R(1) + xp * xp) / d - R(2) * xp * xp * yp * yp / (d * d)) * Yf * Yf;   // (15a)
+  z.Py = z.Py - b * xp / d * Yf;                                                  // (15d)
+  z.T = z.T - b * (R(1) / ref.beta0 + z.Pt) * xp / (R(2) * ps2) * (R(1) - yp * yp) / (d * d) * Yf * Yf;   // (15e)
+  z.Y = Yf;
+  return true;
+}
+// dynamic rotation by phi about y-hat (16)(17) P:228-248 ("P_z" of (17c) read as P_s, A1; the sign of (17e)
+// is the one Hamilton's equations of (16) give, dT/dphi = dH/dPt = -X (1/beta_o + Pt)/P_s, as in (31e): A5),
+// and the passive rotation of the spin components into the new frame
+template <class R> bool rbend_rotate(Particle<R>& p, R phi, const Reference<R>& ref) {
+  Orbit<R>& z = p.z;
+  R ps2 = Ps2(z, ref);
+  if (ps2 <= R(0)) return false;
+  R Ps = m::sqrt(ps2);
+  R c = m::cos(phi), sn = m::sin(phi), t = sn / c;
+  R den = R(1) - z.Px / Ps * t;
+  if (den <= R(0)) return false;
+  R q = z.X * t / den;
+  z.Y = z.Y + z.Py / Ps * q;                                                      // (17c)
+  z.T = z.T - (R(1) / ref.beta0 + z.Pt) / Ps * q;                                 // (17e), sign per A5
+  z.X = z.X / (c * den);                                                          // (17a)
+  z.Px = z.Px * c + Ps * sn;                                                      // (17b)
+  R Sx = p.S.x * c + p.S.s * sn, Ss = -p.S.x * sn + p.S.s * c;                    // same rotation as (Px, Ps)
+  p.S.x = Sx; p.S.s = Ss;
+  return true;
+}
+// fringe spin kick of a rectangular bend (42) P:567 = (41) with m = 1 plus the x-hat term; DESIGN.md reading
+// R10: the printed x-hat term lacks a length -- T-BMT in the fringe's longitudinal field gives
+// (+-b_1/(B rho)_o) G(gamma-1) P_x Y x-hat.
+template <class R> Vec3<R> rbend_fringe_rotvec(const Orbit<R>& z, R sign, R k0, double G, const Reference<R>& ref) {
+  R gamma = ref.gamma0 * (R(1) + ref.beta0 * z.Pt);
+  R b = sign * k0;
+  return Vec3<R>{b * R(G) * (gamma - R(1)) * z.Px * z.Y, R(0), -b * R(1.0 + G) * z.Y};
+}
+
 // ---- solenoid (section 3.7).  e.k0 holds b_0/(B rho)_o, so eta = e.k0/2 (35); (e/p_o) A = eta (-Y, X) (32) ----
 // kinetic transverse momenta (36): canonical minus `frac` times the vector potential
 template <class R> Orbit<R> solenoid_kinetic(const Orbit<R>& z, R eta, R frac) {
@@ -538,6 +600,42 @@ template <class R> bool track_element(Particle<R>& p, const Element& e, Referenc
       if (ok) p.S = quat_rotate(romberg_quaternion(Om, N, ds, depth), p.S);
       break;
     }
+    case RBEND: {
+      // rotate into the magnet frame by phi_entr, entrance fringe (spin kick (42), orbit map (15)),
+      // body (13) in N slices with the edge scheme (Cartesian frame: h = 0 in (6b)), exit fringe, offset (18),
+      // rotate out by -phi_exit, and T_o of (19) so that T stays a deviation.
+      const R k0 = R(e.k0), phi_in = R(e.kn[0]), phi_out = R(e.kn[1]);
+      int N = n_slices * e.slice_mult;
+      R ds = R(e.L) / R(N);
+      const Vec3<R> bfield = {R(0), k0, R(0)};
+      ok = rbend_rotate(p, phi_in, ref);
+      if (!ok) break;
+      p.S = quat_rotate(quat_from_rotvec(rbend_fringe_rotvec(p.z, R(1), k0, G, ref)), p.S);
+      ok = rbend_fringe(p.z, R(1), k0, ref);
+      if (!ok) break;
+      if (depth <= 0) {
+        for (int i = 0; ok && i < N; ++i) {
+          Vec3<R> Om;
+          ok = rbend_body(p.z, ds / R(2), k0, ref) && omega_tbmt(p.z, R(0), bfield, G, ref, Om);
+          if (!ok) break;
+          p.S = quat_rotate(quat_from_rotvec(Vec3<R>{ds * Om.x, ds * Om.y, ds * Om.s}), p.S);
+          ok = rbend_body(p.z, ds / R(2), k0, ref);
+        }
+      } else {
+        std::vector<Vec3<R>> Om(N + 1);
+        ok = omega_tbmt(p.z, R(0), bfield, G, ref, Om[0]);
+        for (int i = 1; ok && i <= N; ++i) ok = rbend_body(p.z, ds, k0, ref) && omega_tbmt(p.z, R(0), bfield, G, ref, Om[i]);
+        if (ok) p.S = quat_rotate(romberg_quaternion(Om, N, ds, depth), p.S);
+      }
+      if (!ok) break;
+      ok = rbend_fringe(p.z, R(-1), k0, ref);
+      if (!ok) break;
+      p.S = quat_rotate(quat_from_rotvec(rbend_fringe_rotvec(p.z, R(-1), k0, G, ref)), p.S);
+      p.z.X = p.z.X - (m::cos(phi_out) - m::cos(phi_in)) / k0;                  // (18): L/(sin - sin) = rho_b
+      ok = rbend_rotate(p, -phi_out, ref);
+      p.z.T = p.z.T + (phi_in - phi_out) / (k0 * ref.beta0);                     // (19): T - T_o, L_arc = rho_b (phi_entr - phi_exit)
+      break;
+    }
     case SOLENOID: {   // entrance fringe kick (40), body (34) in N exact slices with the edge scheme (38)(39), exit kick
       const R eta = R(e.k0) / R(2);
       int N = n_slices * e.slice_mult;
@@ -605,7 +703,8 @@ template <class R> bool track_element(Particle<R>& p, const Element& e, Referenc
 
 inline double ring_circumference(const Element* el, size_t n) {
   double C = 0;
-  for (size_t i = 0; i < n; ++i) C += el[i].L;
+  for (size_t i = 0; i < n; ++i)     // design path length: L, except the arc rho_b (phi_entr - phi_exit) of a rectangular bend (19)
+    C += el[i].type == RBEND ? (el[i].kn[0] - el[i].kn[1]) / el[i].k0 : el[i].L;
   return C;
 }
 

@@ -11,7 +11,7 @@ import numpy as np
 
 from . import build as _build
 
-DRIFT, SBEND, QUAD, MULTIPOLE, THINMULT, RFCAV, SNAKE, MARKER, FRINGE, SOLENOID = range(10)
+DRIFT, SBEND, QUAD, MULTIPOLE, THINMULT, RFCAV, SNAKE, MARKER, FRINGE, SOLENOID, RBEND = range(11)
 SPLIT_DRIFT_KICK, SPLIT_BEND_KICK, SPLIT_MATRIX_KICK = range(3)
 PREC_DOUBLE, PREC_LONG_DOUBLE, PREC_QUAD = range(3)
 

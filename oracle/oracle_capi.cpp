@@ -51,14 +51,14 @@ int validate(const Element* el, size_t n_el, int split, int n_slices, int depth)
   if (n_slices < 1 || depth < -1 || depth > 12 || split < 0 || split > 5) return 1;   // depth 0, -1: PWC (section 4.1)
   for (size_t e = 0; e < n_el; ++e) {
     int t = el[e].type;
-    if (t < 0 || t > SOLENOID) return 1;
-    if (t == SBEND || t == QUAD || t == MULTIPOLE || t == SOLENOID) {
+    if (t < 0 || t > RBEND) return 1;
+    if (t == SBEND || t == QUAD || t == MULTIPOLE || t == SOLENOID || t == RBEND) {
       if (el[e].slice_mult < 1 || el[e].L == 0) return 1;   // L < 0 allowed here: inverse flow, used by the reversibility pins
       long N = (long)n_slices * el[e].slice_mult;
       if (depth >= 1 && N % (1L << (depth - 1)) != 0) return 1;   // A4
       if (t == SBEND && (el[e].h == 0 || el[e].k0 == 0)) return 1;
       if (t == QUAD && el[e].kn[0] == 0) return 1;
-      if (t == SOLENOID && el[e].k0 == 0) return 1;
+      if ((t == SOLENOID || t == RBEND) && el[e].k0 == 0) return 1;
     }
   }
   return 0;

@@ -15,7 +15,7 @@ import math
 
 import numpy as np
 
-DRIFT, SBEND, QUAD, MULTIPOLE, THINMULT, RFCAV, SNAKE, MARKER, FRINGE, SOLENOID = range(10)
+DRIFT, SBEND, QUAD, MULTIPOLE, THINMULT, RFCAV, SNAKE, MARKER, FRINGE, SOLENOID, RBEND = range(11)
 SPLIT_DRIFT_KICK, SPLIT_BEND_KICK, SPLIT_MATRIX_KICK = range(3)
 # the same splits with the fourth-order composition of every non-exact slice map (gst.h)
 SPLIT_DRIFT_KICK_4, SPLIT_BEND_KICK_4, SPLIT_MATRIX_KICK_4 = range(3, 6)
@@ -119,6 +119,21 @@ def solenoid(L, ks, slice_mult=1):
     return e
 
 
+def rbend(L, angle, phi_entr=None, phi_exit=None, slice_mult=1):
+    """Rectangular bend (section 3.2): magnet length L along its axis, total bend angle; the beam meets the
+    entrance face at phi_entr and leaves at phi_exit (default symmetric: +-angle/2); sin(phi_entr) -
+    sin(phi_exit) = L/rho_b fixes the field k0 = 1/rho_b (13b)."""
+    if phi_entr is None:
+        phi_entr, phi_exit = 0.5 * angle, -0.5 * angle
+    assert abs((phi_entr - phi_exit) - angle) < 1e-15 * max(1.0, abs(angle))
+    e = _blank(RBEND)
+    e["L"] = L
+    e["k0"] = (math.sin(phi_entr) - math.sin(phi_exit)) / L
+    e["kn"] = (phi_entr, phi_exit, 0.0, 0.0)
+    e["slice_mult"] = slice_mult
+    return e
+
+
 def with_fringes(magnet):
     """[entrance fringe, magnet, exit fringe] for a thick SBEND / QUAD / MULTIPOLE element."""
     k0 = float(magnet["k0"]) if int(magnet["type"]) == SBEND else 0.0
@@ -140,7 +155,7 @@ def beta_of_gamma(g):
 
 def steps_per_turn(lat, n_slices):
     """particle-element-steps per particle per turn."""
-    thick = np.isin(lat["type"], (SBEND, QUAD, MULTIPOLE, SOLENOID))
+    thick = np.isin(lat["type"], (SBEND, QUAD, MULTIPOLE, SOLENOID, RBEND))
     return int(np.sum(np.where(thick, n_slices * lat["slice_mult"], 1)))
 
 
