@@ -42,10 +42,15 @@ typedef enum {
                         (m = 2..5, per unit length): rotation about s-hat by
                         -sign (1+G) [k0 Y + sum_m (kn Im (X+iY)^m + ks Re (X+iY)^m)/m]; sign = +1 at the
                         entrance, -1 at the exit; orbit-transparent (the paper gives no orbital fringe map)  */
-  GST_SOLENOID = 9   /* solenoid with thin-pancake fringes, section 3.7: k0 = b_0/(B rho)_o [1/m] (eta of (35)
+  GST_SOLENOID = 9,  /* solenoid with thin-pancake fringes, section 3.7: k0 = b_0/(B rho)_o [1/m] (eta of (35)
                         is k0/2), L > 0; exact body flow (34) in n_slices*slice_mult slices for the spin scheme, Omega
                         with u-hat from the kinetic momentum (36), fringe spin kicks (40) at both ends; the orbit is
                         canonical throughout (the fringes leave the canonical momenta unchanged)             */
+  GST_RBEND = 10     /* rectangular bend, section 3.2: L = magnet length along its axis, k0 = b_1/(B rho)_o =
+                        1/rho_b, kn[0] = phi_entr, kn[1] = phi_exit (angles between the design orbit and the normals of
+                        the two faces; sin(phi_entr) - sin(phi_exit) = L*k0, else GST_EINVAL).  Rotation (17) into the
+                        magnet frame, fringe spin kick (42) and orbit map (15), body (13) in n_slices*slice_mult slices,
+                        exit fringe, offset (18), rotation out, time offset (19)                                     */
 } gst_elem_type;
 
 /* which integrator each thick magnet uses (".apdf"; reading A16).  The *_4 values take the

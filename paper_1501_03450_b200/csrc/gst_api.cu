@@ -39,7 +39,7 @@ gst_status fail(gst_status s, const char* fmt, ...) {
     if (e_ != cudaSuccess) return fail(GST_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
   } while (0)
 
-bool is_thick(int t) { return t == GST_SBEND || t == GST_QUAD || t == GST_MULTIPOLE || t == GST_SOLENOID; }
+bool is_thick(int t) { return t == GST_SBEND || t == GST_QUAD || t == GST_MULTIPOLE || t == GST_SOLENOID || t == GST_RBEND; }
 
 struct DevTable {
   gst::DevElem* d_tab = nullptr;
@@ -135,6 +135,26 @@ gst::DevElem derive(const gst_element& e, int n_slices, double C) {
     d.dEs = e.volt_eV * std::sin(e.phi_s);
   }
   if (e.type == GST_FRINGE) d.sign = e.sign;
+  if (e.type == GST_RBEND) {
+    const long double ang[2] = {(long double)e.kn[0], -(long double)e.kn[1]};
+    for (int k = 0; k < 2; ++k) {
+      d.rb_c[k] = (double)cosl(ang[k]);
+      d.rb_s[k] = (double)sinl(ang[k]);
+      d.rb_t[k] = (double)tanl(ang[k]);
+      d.rb_sec[k] = (double)(1.0L / cosl(ang[k]));
+      d.rb_qw[k] = (double)cosl(0.5L * ang[k]);
+      d.rb_qy[k] = (double)sinl(0.5L * ang[k]);
+    }
+    const long double rho = 1.0L / (long double)e.k0, dphi = (long double)e.kn[0] - (long double)e.kn[1];
+    d.rb_rho = (double)rho;
+    d.rb_xoff = (double)(rho * (cosl(e.kn[1]) - cosl(e.kn[0])));
+    d.rb_arc = (double)(rho * dphi);
+    d.rb_cd = (double)cosl(dphi);
+    d.rb_sd = (double)sinl(dphi);
+    d.kn[0] = d.kn[1] = 0.0;          // the angles are not multipole strengths
+    d.order = 2;
+    d.pure_quad = 0;
+  }
   if (e.type == GST_SNAKE) {
     double sh = std::sin(0.5 * e.snake_mu);
     d.qw = std::cos(0.5 * e.snake_mu);
@@ -268,11 +288,16 @@ gst_status gst_lattice_create(const gst_element* elems, size_t n, const gst_beam
   if (!(beam->gamma0 > 1.0) || !(beam->mass_eV > 0.0)) return fail(GST_EINVAL, "beam: need gamma0 > 1 and mass_eV > 0");
   for (size_t i = 0; i < n; ++i) {
     const gst_element& e = elems[i];
-    if (e.type < 0 || e.type > GST_SOLENOID) return fail(GST_EINVAL, "element %zu: unknown type %d", i, e.type);
+    if (e.type < 0 || e.type > GST_RBEND) return fail(GST_EINVAL, "element %zu: unknown type %d", i, e.type);
     if ((is_thick(e.type) || e.type == GST_DRIFT) && !(e.L > 0.0)) return fail(GST_EINVAL, "element %zu: L must be > 0", i);
     if (is_thick(e.type) && e.slice_mult < 1) return fail(GST_EINVAL, "element %zu: slice_mult must be >= 1", i);
     if (e.type == GST_SBEND && (e.h == 0.0 || e.k0 == 0.0)) return fail(GST_EINVAL, "element %zu: SBEND needs h != 0 and k0 != 0", i);
     if (e.type == GST_SOLENOID && e.k0 == 0.0) return fail(GST_EINVAL, "element %zu: SOLENOID needs k0 != 0", i);
+    if (e.type == GST_RBEND) {
+      if (e.k0 == 0.0) return fail(GST_EINVAL, "element %zu: RBEND needs k0 != 0", i);
+      if (std::fabs(std::sin(e.kn[0]) - std::sin(e.kn[1]) - e.L * e.k0) > 1e-12 * (1.0 + std::fabs(e.L * e.k0)))
+        return fail(GST_EINVAL, "element %zu: RBEND needs sin(phi_entr) - sin(phi_exit) = L*k0 (13b)", i);
+    }
     if (e.type == GST_QUAD) {
       if (e.kn[0] == 0.0) return fail(GST_EINVAL, "element %zu: QUAD needs kn[0] != 0", i);
       for (int k = 0; k < 4; ++k)
@@ -287,7 +312,9 @@ gst_status gst_lattice_create(const gst_element* elems, size_t n, const gst_beam
   for (size_t i = 0; i < n; ++i) {
     gst_element e = elems[i];
     if (!is_thick(e.type)) e.slice_mult = 1;
-    if (e.type == GST_DRIFT || is_thick(e.type)) lat->C += e.L; else e.L = 0.0;
+    if (e.type == GST_RBEND) lat->C += (e.kn[0] - e.kn[1]) / e.k0;   // design arc length (19)
+    else if (e.type == GST_DRIFT || is_thick(e.type)) lat->C += e.L;
+    else e.L = 0.0;
     size_t k = 0;
     for (; k < lat->uniq.size(); ++k)
       if (std::memcmp(&lat->uniq[k], &e, sizeof e) == 0) break;

@@ -21,7 +21,7 @@
 
 namespace gst {
 
-enum : int { K_DRIFT = 0, K_SBEND = 1, K_QUAD = 2, K_MULT = 3, K_THIN = 4, K_RF = 5, K_SNAKE = 6, K_MARKER = 7, K_FRINGE = 8, K_SOLENOID = 9 };
+enum : int { K_DRIFT = 0, K_SBEND = 1, K_QUAD = 2, K_MULT = 3, K_THIN = 4, K_RF = 5, K_SNAKE = 6, K_MARKER = 7, K_FRINGE = 8, K_SOLENOID = 9, K_RBEND = 10 };
 enum : int { SPLIT_DK = 0, SPLIT_BK = 1, SPLIT_MK = 2 };
 
 // Fourth-order symmetric composition of a second-order slice map S2 (R5):
@@ -61,6 +61,13 @@ struct __align__(16) DevElem {
   // (x1 + x0) ds/2 < 0 (the merged neighbours of the fourth-order composition, see Yoshida above), [3] over ds
   // (the whole drifts of the DKSKD ordering, whose table is derived for half slices)
   TeapotHalf th[4];
+  // rectangular bend (section 3.2): rotations (17) by phi_entr [0] and by -phi_exit [1]
+  double rb_c[2], rb_s[2], rb_t[2], rb_sec[2];   // cos, sin, tan, sec of the rotation angle
+  double rb_qw[2], rb_qy[2];                     // the same rotation of the spin components: (cos, sin)(angle/2) about y
+  double rb_rho;                                 // rho_b = 1/k0 (12)
+  double rb_xoff;                                // (18): rho_b (cos phi_exit - cos phi_entr)
+  double rb_arc;                                 // rho_b (phi_entr - phi_exit), (19)
+  double rb_cd, rb_sd;                           // cos, sin of phi_entr - phi_exit
   double kn[4], ks[4]; // multipole strengths (28); thin: integrated
   // cavity
   double volt, krf_over_beta, phi_s, sign, dEs;
@@ -464,15 +471,9 @@ struct BendExact {
 
 __constant__ double APOLY[6] = {1.0 / 6.0, 3.0 / 40.0, 15.0 / 336.0, 105.0 / 3456.0, 945.0 / 42240.0, 10395.0 / 599040.0};
 
-template <class Spin>
-__device__ __forceinline__ bool sbend_exact(State& z, const DevElem& e, const PCon& c, const Ref& r, Spin& spin) {
-  BendExact s(z, e, c);
-  const double A0 = s.A, Am1_0 = s.Am1, Px0 = z.Px;
-  spin.run(s, e.N, e.ds);
-  // asin(Px0/Pa) - asin(PxN/Pa) = asin(x),  x = (Px0 A_N - Px_N A_0)/Pa^2  (no cancellation)
-  const double x = fma(Px0, s.Am1 - Am1_0, -(z.Px - Px0) * A0) * rcp_nr(s.Pa2);
+// asin(x): polynomial for the small arguments of differences of nearby angles, the library routine otherwise
+__device__ __forceinline__ double asin_small(double x) {
   const double v = x * x;
-  double dasin;
   if (v < 2.5e-3) {     // asin(x)/x = 1 + v/6 + 3v^2/40 + 15v^3/336 + 105v^4/3456 + 945v^5/42240 + 10395v^6/599040
     double p = APOLY[5];
     p = fma(p, v, APOLY[4]);
@@ -480,10 +481,19 @@ __device__ __forceinline__ bool sbend_exact(State& z, const DevElem& e, const PC
     p = fma(p, v, APOLY[2]);
     p = fma(p, v, APOLY[1]);
     p = fma(p, v, APOLY[0]);
-    dasin = fma(p * v, x, x);
-  } else {
-    dasin = asin(x);
+    return fma(p * v, x, x);
   }
+  return asin(x);
+}
+
+template <class Spin>
+__device__ __forceinline__ bool sbend_exact(State& z, const DevElem& e, const PCon& c, const Ref& r, Spin& spin) {
+  BendExact s(z, e, c);
+  const double A0 = s.A, Am1_0 = s.Am1, Px0 = z.Px;
+  spin.run(s, e.N, e.ds);
+  // asin(Px0/Pa) - asin(PxN/Pa) = asin(x),  x = (Px0 A_N - Px_N A_0)/Pa^2  (no cancellation)
+  const double x = fma(Px0, s.Am1 - Am1_0, -(z.Px - Px0) * A0) * rcp_nr(s.Pa2);
+  const double dasin = asin_small(x);
   const double dh = dasin * e.inv_h;
   z.Y = fma(z.Py * e.inv_eta, e.L + dh, z.Y);
   z.T += e.inv_eta * (fma(-z.Pt, e.L, -c.ibpt * dh) - e.ome * e.L * r.ibeta0);
@@ -830,6 +840,101 @@ __device__ __forceinline__ bool quad_mk(State& z, const DevElem& e, const PCon& 
 // ---------------------------------------------------------------------------------------------
 // one element (the dispatch is uniform across the grid: every particle is in the same element)
 // ---------------------------------------------------------------------------------------------
+// f3: rectangular bend (section 3.2).  e.k0 = 1/rho_b; all coordinates between the two rotations are
+// internal to the magnet (Cartesian frame along its axis).
+struct BendRect {     // body (13): Px falls linearly, X follows sqrt(Pa^2 - Px^2); Y, T once per element
+  State& z;
+  double k0, ds, Pa2, A, iA, q2, a1k;
+  bool bad;
+  __device__ __forceinline__ BendRect(State& z_, const DevElem& e, const PCon& c) : z(z_), k0(e.k0), ds(e.ds) {
+    Pa2 = fma(-z.Py, z.Py, 1.0 + c.e0);                    // (8)
+    const double a2 = fma(-z.Px, z.Px, Pa2);
+    bad = !(a2 > 0.0);
+    iA = rsqrt_nr(a2);
+    A = a2 * iA;
+    q2 = c.a2p * e.k0 * z.Py;
+    a1k = fma(c.a1, e.k0, -q2 * z.Py);
+  }
+  __device__ __forceinline__ void advance() {
+    const double Pxf = fma(-ds, k0, z.Px);                 // (13b)
+    const double f2 = fma(-Pxf, Pxf, Pa2);
+    bad |= !(f2 > 0.0);
+    const double y = rsqrt_nr(f2);
+    const double Af = f2 * y;
+    // (13a): rho_b (A_f - A) = rho_b (Px - Px_f)(Px + Px_f)/(A_f + A) = ds (Px + Px_f)/(A_f + A)
+    z.X = fma(ds * (z.Px + Pxf), rcp_nr(Af + A), z.X);
+    z.Px = Pxf; A = Af; iA = y;
+  }
+  template <bool DKSKD> __device__ __forceinline__ void pwc_first() { advance(); }
+  template <bool DKSKD> __device__ __forceinline__ void pwc_second() { advance(); }
+  // (6b) with h = 0, b = (0, k0, 0), Ps = A
+  __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) const {
+    const double fw = iA * w;
+    const double fq = fw * q2;
+    wx = fq * z.Px;
+    wy = -fw * a1k;
+    ws = fq * A;
+  }
+};
+// dynamic rotation (17) about y-hat; k = 0: by phi_entr, k = 1: by -phi_exit (constants from the host)
+__device__ __forceinline__ bool rbend_rotate(State& z, const DevElem& e, int k, const PCon& c) {
+  const double ps2 = 1.0 + c.e0 - fma(z.Px, z.Px, z.Py * z.Py);
+  const double iPs = rsqrt_nr(ps2);
+  const double Ps = ps2 * iPs;
+  const double den = fma(-z.Px * iPs, e.rb_t[k], 1.0);
+  const double q = z.X * e.rb_t[k] * rcp_nr(den);
+  z.Y = fma(z.Py * iPs, q, z.Y);                           // (17c)
+  z.T = fma(-c.ibpt * iPs, q, z.T);                        // (17e), sign of reading A5
+  z.X = z.X * e.rb_sec[k] * rcp_nr(den);                   // (17a)
+  z.Px = fma(z.Px, e.rb_c[k], Ps * e.rb_s[k]);             // (17b)
+  return ps2 > 0.0 && den > 0.0;
+}
+// thin-fringe orbit map (15), b = +-k0
+__device__ __forceinline__ bool rbend_fringe(State& z, double b, const PCon& c) {
+  const double ps2 = 1.0 + c.e0 - fma(z.Px, z.Px, z.Py * z.Py);
+  const double iPs = rsqrt_nr(ps2);
+  const double xp = z.Px * iPs, yp = z.Py * iPs;
+  const double id = rcp_nr(fma(yp, yp, 1.0));
+  const double arg = fma(2.0 * b * xp * yp * id, z.Y, 1.0);
+  const double Yf = 2.0 * z.Y * rcp_nr(1.0 + arg * rsqrt_nr(arg));                                  // (15c)
+  const double Y2 = Yf * Yf;
+  z.X = fma(0.5 * b * iPs * (fma(xp, xp, 1.0) * id - 2.0 * xp * xp * yp * yp * id * id), Y2, z.X);  // (15a)
+  z.Py = fma(-b * xp * id, Yf, z.Py);                                                               // (15d)
+  z.T = fma(-0.5 * b * c.ibpt * xp * iPs * iPs * fma(-yp, yp, 1.0) * id * id, Y2, z.T);             // (15e)
+  z.Y = Yf;
+  return ps2 > 0.0 && arg > 0.0;
+}
+template <class Spin>
+__device__ __forceinline__ bool rbend(State& z, const DevElem& e, const PCon& c, const Ref& r, double G, Spin& spin) {
+  bool ok = rbend_rotate(z, e, 0, c);
+  spin.snake(Quat{e.rb_qw[0], 0.0, e.rb_qy[0], 0.0});
+  const double g1 = c.a2p * (1.0 + c.e0);                   // G (gamma - 1)
+  // entrance: spin kick (42) (with the length Y in its x-hat term, R10), then the orbit map (15)
+  spin.thin(e.k0 * g1 * z.Px * z.Y, 0.0, -e.k0 * (1.0 + G) * z.Y);
+  ok &= rbend_fringe(z, e.k0, c);
+  BendRect s(z, e, c);
+  const double A0 = s.A, Px0 = z.Px;
+  spin.run(s, e.N, e.ds);
+  {   // Y (13c) and T (13e) + (19) over the whole body.  d = asin(Px0/Pa) - asin(PxN/Pa):
+      //   sin d = (Px0 A_N - Px_N A_0)/Pa^2,  cos d = (A_0 A_N + Px0 Px_N)/Pa^2;
+      // delta = d - (phi_entr - phi_exit) from sin delta = sin d cos D - cos d sin D, so that
+      //   T: -(1/beta_o + Pt) rho_b d + L_arc/beta_o = -(1/beta_o + Pt) rho_b delta - Pt L_arc   (no O(1) cancellation)
+    const double iPa2 = rcp_nr(s.Pa2);
+    const double sd = fma(Px0, s.A, -z.Px * A0) * iPa2, cd = fma(A0, s.A, Px0 * z.Px) * iPa2;
+    const double delta = asin_small(fma(sd, e.rb_cd, -cd * e.rb_sd));
+    z.Y = fma(z.Py, fma(e.rb_rho, delta, e.rb_arc), z.Y);
+    z.T = fma(-c.ibpt * e.rb_rho, delta, fma(-z.Pt, e.rb_arc, z.T));
+  }
+  ok &= !s.bad;
+  ok &= rbend_fringe(z, -e.k0, c);
+  spin.thin(-e.k0 * g1 * z.Px * z.Y, 0.0, e.k0 * (1.0 + G) * z.Y);
+  z.X -= e.rb_xoff;                                         // (18)
+  ok &= rbend_rotate(z, e, 1, c);
+  spin.snake(Quat{e.rb_qw[1], 0.0, e.rb_qy[1], 0.0});
+  (void)r;
+  return ok;
+}
+
 // f4: solenoid with thin-pancake fringes (section 3.7).  e.k0 = b_0/(B rho)_o, eta = k0/2 (35).
 // The body flow (34) is exact, so a slice is the same map over ds; Ps of (33) is an invariant of it, which
 // makes kappa = eta/Ps and cos/sin(kappa ds) per-particle constants of the element, and lets T (34c) be
@@ -944,6 +1049,7 @@ __device__ __forceinline__ bool element_step(int type, State& z, const DevElem& 
   }
   if (type == K_SNAKE) spin.snake(Quat{e.qw, e.qx, e.qy, e.qs});
   if (type == K_SOLENOID) return solenoid(z, e, pc, ref, spin);
+  if (type == K_RBEND) return rbend(z, e, pc, ref, G, spin);
   if (type == K_FRINGE) {   // thin-fringe spin kick (41) P:561: rotation about s-hat, orbit untouched
     double re = z.X, im = z.Y;                       // (X + iY)^m
     double psi = e.k0 * im;                          // m = 1

@@ -195,6 +195,14 @@ __device__ __forceinline__ void spin_role(const TrackArgs& a, const DevElem* tab
       const int type = (int)(cur & 0xffu);
       if (type == K_SBEND || type == K_QUAD || type == K_MULT) {
         spin.template thick<DEPTH>(e.N, Sx, Sy, Ss);
+      } else if (type == K_RBEND) {               // frame rotation, fringe kick, body, fringe kick, frame rotation
+        quat_rotate(Quat{e.rb_qw[0], 0.0, e.rb_qy[0], 0.0}, Sx, Sy, Ss);
+        Quat q = spin.pop();
+        quat_rotate(q, Sx, Sy, Ss);
+        spin.template thick<DEPTH>(e.N, Sx, Sy, Ss);
+        q = spin.pop();
+        quat_rotate(q, Sx, Sy, Ss);
+        quat_rotate(Quat{e.rb_qw[1], 0.0, e.rb_qy[1], 0.0}, Sx, Sy, Ss);
       } else if (type == K_SOLENOID) {            // entrance kick, body, exit kick
         Quat q = spin.pop();
         quat_rotate(q, Sx, Sy, Ss);

@@ -216,6 +216,28 @@ def test_solenoids_in_a_ring(gst, O, variant, depth, n_slices):
     assert orbit_err(got, ref) < 2e-12 and spin_err(got, ref) < 2e-12, (orbit_err(got, ref), spin_err(got, ref))
 
 
+@pytest.mark.parametrize("variant,depth,n_slices", [("fused", 1, 3), ("fused", 4, 8), ("fused", 6, 32), ("pair", 3, 4),
+                                                    ("fused", W.PWC_HALF_SLICE, 4), ("fused", W.PWC_DKSKD, 4)])
+def test_rectangular_bends_in_a_ring(gst, O, variant, depth, n_slices):
+    """GST_RBEND: rotations (17), fringe map (15) and spin kick (42), body (13), offsets (18)(19)."""
+    els = list(mixed_lattice())
+    els.insert(2, W.rbend(2.4, 0.12))                         # symmetric
+    els.insert(15, W.rbend(1.6, 0.09, 0.07, -0.02, slice_mult=2))   # asymmetric: offset (18)
+    els.insert(30, W.rbend(2.0, -0.08))                       # bends the other way
+    lat = W.lattice(els)
+    bm = W.beam(12.0)
+    st = W.gaussian_bunch(23, 200, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
+    ref, rlost, g_ref = O.track(lat, bm, st, 2, W.SPLIT_BEND_KICK, n_slices, depth)
+    try:
+        gst.set_kernel_variant(gst.KERNEL_PAIR if variant == "pair" else gst.KERNEL_FUSED)
+        got, lost, pol, emit, g_gpu = gpu_track(gst, lat, bm, st, 2, W.SPLIT_BEND_KICK, n_slices, depth)
+    finally:
+        gst.set_kernel_variant(gst.KERNEL_FUSED)
+    assert not rlost.any() and not lost.any()
+    assert orbit_err(got, ref) < 2e-12 and spin_err(got, ref) < 2e-12, (orbit_err(got, ref), spin_err(got, ref))
+    assert abs(g_gpu - g_ref) < 1e-12 * g_ref                 # the cavity sees the same circumference (arc lengths)
+
+
 def test_large_angle_per_slice_takes_the_sincos_branch(gst, O):
     # one slice through a strong bend at high G*gamma: rotation angle per edge > 1.4 rad
     lat = W.lattice([W.sbend(9.45, 0.2), W.drift(1.0)])
