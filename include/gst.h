@@ -136,10 +136,14 @@ gst_status gst_track_pwc(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, 
                          gst_pwc_order order, void* cuda_stream);
 
 /* Which tracking kernel gst_track launches (process-wide; results are bit-identical):
- *   GST_KERNEL_FUSED  one thread per particle, orbit and spin work software-pipelined -- default
- *   GST_KERNEL_PAIR   experimental: an orbit thread and a spin thread per particle, coupled through a
- *                     shared-memory ring (csrc/track_pair_kernel.cuh); slower on B200 as measured      */
-typedef enum { GST_KERNEL_FUSED = 0, GST_KERNEL_PAIR = 1 } gst_kernel_variant;
+ *   GST_KERNEL_FUSED         one thread per particle, orbit and spin work software-pipelined -- default.
+ *                            When the bunch fits the chip in one wave but fills its sub-partitions unevenly (e.g.
+ *                            65 536 particles = 3.46 warps each), the turns are cut into chunks and the warps of
+ *                            particles rotate over all resident warp slots (csrc/track_chain_kernel.cuh)
+ *   GST_KERNEL_FUSED_STATIC  the same kernel without the rotation: every warp keeps its slot for the whole call
+ *   GST_KERNEL_PAIR          experimental: an orbit thread and a spin thread per particle, coupled through a
+ *                            shared-memory ring (csrc/track_pair_kernel.cuh); slower on B200 as measured      */
+typedef enum { GST_KERNEL_FUSED = 0, GST_KERNEL_PAIR = 1, GST_KERNEL_FUSED_STATIC = 2 } gst_kernel_variant;
 gst_status gst_set_kernel_variant(gst_kernel_variant v);
 
 /* Bunch polarization (a13; reading A18): out = {Px, Py, Ps, |P|} over particles not lost;

@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <algorithm>
 #include <atomic>
 #include <cstdarg>
 #include <cstdio>
@@ -18,6 +19,7 @@
 #include "reduce_kernel.cuh"
 #include "track_kernel.cuh"
 #include "track_pair_kernel.cuh"
+#include "track_chain_kernel.cuh"
 
 namespace {
 
@@ -69,6 +71,10 @@ struct gst_bunch {
   bool have_ref = false;
   double E0 = 0, mass = 0;
   int64_t turn = 0;
+  // chain rotation (track_chain_kernel.cuh): per-chain progress flags and reference energies, error word
+  int* d_chain_flag = nullptr;
+  double* d_chain_E0 = nullptr;
+  int* d_err = nullptr;
 };
 
 namespace {
@@ -204,8 +210,23 @@ SmemPlan plan_smem(size_t tab_bytes, size_t seq_bytes, size_t fixed, size_t budg
   return p;
 }
 
+// Does rotating the chains over the warp slots pay (track_chain_kernel.cuh)?  Only when the bunch fits the chip in
+// one wave but fills its sub-partitions unevenly, and there are enough turns to cut into chunks.
+bool chain_plan(long long n, long long n_turns, int slots, int sms, gst::ChainArgs* ch) {
+  const long long n_chains = (n + 31) / 32;
+  const long long smsp = 4LL * sms;
+  if (n_chains > slots || n_turns < 16 || 2 * n_chains < 3 * smsp) return false;
+  const long long maxw = (n_chains + smsp - 1) / smsp;
+  if ((double)maxw * smsp < 1.04 * (double)n_chains) return false;      // already even
+  ch->n_chains = (int)n_chains;
+  ch->chunk_turns = (int)std::max<long long>(1, n_turns / 24);
+  ch->shift = (slots - (int)n_chains) & ~1;
+  return ch->shift > 0;
+}
+
 template <int SPLIT, int DEPTH, int ORDER>
-cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, bool pair, cudaStream_t st) {
+cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, bool pair, cudaStream_t st,
+                         gst::ChainArgs* chain = nullptr) {
   if constexpr (ORDER == 2 && DEPTH >= 1) {   // the experimental pair kernel: second-order maps, edge scheme only
   if (pair) {
     // T1p: two threads per particle.  Shared memory per block is budgeted so that MIN_BLOCKS blocks stay
@@ -230,10 +251,29 @@ cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, b
     return cudaGetLastError();
   }
   }
-  // T1: one thread per particle; shared memory kept small so that 8 blocks of 64 threads stay resident
-  auto kern = gst::track_kernel<SPLIT, DEPTH, ORDER>;
   SmemPlan p = plan_smem(tab_bytes, seq_bytes, 0, 24 * 1024);
   a.use_smem_seq = p.use_smem_seq;
+  if constexpr (ORDER == 2 && DEPTH >= 1) {
+    if (chain) {   // T1c: the same kernel with the chains rotating over all resident warp slots
+      auto ck = gst::track_chain_kernel<SPLIT, DEPTH, ORDER>;
+      int dev = 0, sms = 0, per_sm = 0;
+      cudaGetDevice(&dev);
+      cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+      if (p.bytes > 48 * 1024) cudaFuncSetAttribute(ck, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
+      cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ck, gst::TRACK_BLOCK, p.bytes);
+      if (e != cudaSuccess) return e;
+      if (per_sm > gst::TRACK_MIN_BLOCKS) per_sm = gst::TRACK_MIN_BLOCKS;
+      const int blocks = per_sm * sms;
+      if (chain_plan(a.n, a.n_turns, blocks * (gst::TRACK_BLOCK / 32), sms, chain)) {
+        e = cudaMemsetAsync(chain->flag, 0, sizeof(int) * chain->n_chains, st);
+        if (e != cudaSuccess) return e;
+        ck<<<blocks, gst::TRACK_BLOCK, p.bytes, st>>>(a, *chain);
+        return cudaGetLastError();
+      }
+    }
+  }
+  // T1: one thread per particle; shared memory kept small so that 8 blocks of 64 threads stay resident
+  auto kern = gst::track_kernel<SPLIT, DEPTH, ORDER>;
   if (p.bytes > 48 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
     if (e != cudaSuccess) return e;
@@ -244,16 +284,17 @@ cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, b
 }
 
 template <int SPLIT, int ORDER>
-cudaError_t launch_track_depth(int depth, const gst::TrackArgs& a, size_t tb, size_t sb, bool pair, cudaStream_t st) {
+cudaError_t launch_track_depth(int depth, const gst::TrackArgs& a, size_t tb, size_t sb, bool pair, cudaStream_t st,
+                               gst::ChainArgs* chain) {
   if (ORDER == 2 && depth == 0) return launch_track<SPLIT, 0, 2>(a, tb, sb, false, st);
   if (ORDER == 2 && depth == -1) return launch_track<SPLIT, -1, 2>(a, tb, sb, false, st);
   switch (depth) {
-    case 1: return launch_track<SPLIT, 1, ORDER>(a, tb, sb, pair, st);
-    case 2: return launch_track<SPLIT, 2, ORDER>(a, tb, sb, pair, st);
-    case 3: return launch_track<SPLIT, 3, ORDER>(a, tb, sb, pair, st);
-    case 4: return launch_track<SPLIT, 4, ORDER>(a, tb, sb, pair, st);
-    case 5: return launch_track<SPLIT, 5, ORDER>(a, tb, sb, pair, st);
-    default: return launch_track<SPLIT, 6, ORDER>(a, tb, sb, pair, st);
+    case 1: return launch_track<SPLIT, 1, ORDER>(a, tb, sb, pair, st, chain);
+    case 2: return launch_track<SPLIT, 2, ORDER>(a, tb, sb, pair, st, chain);
+    case 3: return launch_track<SPLIT, 3, ORDER>(a, tb, sb, pair, st, chain);
+    case 4: return launch_track<SPLIT, 4, ORDER>(a, tb, sb, pair, st, chain);
+    case 5: return launch_track<SPLIT, 5, ORDER>(a, tb, sb, pair, st, chain);
+    default: return launch_track<SPLIT, 6, ORDER>(a, tb, sb, pair, st, chain);
   }
 }
 
@@ -278,7 +319,7 @@ extern "C" {
 const char* gst_last_error(void) { return g_err.c_str(); }
 
 gst_status gst_set_kernel_variant(gst_kernel_variant v) {
-  if (v != GST_KERNEL_FUSED && v != GST_KERNEL_PAIR) return fail(GST_EINVAL, "unknown kernel variant %d", (int)v);
+  if (v != GST_KERNEL_FUSED && v != GST_KERNEL_PAIR && v != GST_KERNEL_FUSED_STATIC) return fail(GST_EINVAL, "unknown kernel variant %d", (int)v);
   g_variant.store((int)v);
   return GST_OK;
 }
@@ -365,6 +406,11 @@ gst_status gst_bunch_init(double* x, double* px, double* y, double* py, double* 
   if (ce == cudaSuccess) ce = cudaMalloc(&b->d_partials, sizeof(double) * gst::RED_MAX_BLOCKS * gst::RED_WIDTH);
   if (ce == cudaSuccess) ce = cudaMalloc(&b->d_result, sizeof(double) * 2 * gst::RED_WIDTH);
   if (ce == cudaSuccess) ce = cudaMallocHost(&b->h_result, sizeof(double) * 2 * gst::RED_WIDTH);
+  const size_t n_chains = (n + 31) / 32 + 1;
+  if (ce == cudaSuccess) ce = cudaMalloc(&b->d_chain_flag, sizeof(int) * n_chains);
+  if (ce == cudaSuccess) ce = cudaMalloc(&b->d_chain_E0, sizeof(double) * n_chains);
+  if (ce == cudaSuccess) ce = cudaMalloc(&b->d_err, sizeof(int));
+  if (ce == cudaSuccess) ce = cudaMemset(b->d_err, 0, sizeof(int));
   if (ce != cudaSuccess) {
     gst_bunch_destroy(b);
     return fail(ce == cudaErrorMemoryAllocation ? GST_ENOMEM : GST_ECUDA, "gst_bunch_init: %s", cudaGetErrorString(ce));
@@ -379,6 +425,9 @@ void gst_bunch_destroy(gst_bunch* b) {
   if (b->d_partials) cudaFree(b->d_partials);
   if (b->d_result) cudaFree(b->d_result);
   if (b->h_result) cudaFreeHost(b->h_result);
+  if (b->d_chain_flag) cudaFree(b->d_chain_flag);
+  if (b->d_chain_E0) cudaFree(b->d_chain_E0);
+  if (b->d_err) cudaFree(b->d_err);
   delete b;
 }
 
@@ -434,16 +483,21 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   size_t seq_bytes = (lat->seq.size() * sizeof(uint32_t) + 15) & ~size_t(15);
   if (tab_bytes > 24 * 1024) return fail(GST_EINVAL, "too many unique elements for the shared-memory table (%zu)", lat->uniq.size());
   const bool pair = g_variant.load() == GST_KERNEL_PAIR;
+  gst::ChainArgs chain_args;
+  chain_args.flag = b->d_chain_flag;
+  chain_args.E0 = b->d_chain_E0;
+  chain_args.err = b->d_err;
+  gst::ChainArgs* chain = g_variant.load() == GST_KERNEL_FUSED ? &chain_args : nullptr;
   a.use_smem_seq = 0;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   cudaError_t ce;
   switch (split) {
-    case GST_SPLIT_DRIFT_KICK: ce = launch_track_depth<gst::SPLIT_DK, 2>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
-    case GST_SPLIT_BEND_KICK: ce = launch_track_depth<gst::SPLIT_BK, 2>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
-    case GST_SPLIT_MATRIX_KICK: ce = launch_track_depth<gst::SPLIT_MK, 2>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
-    case GST_SPLIT_DRIFT_KICK_4: ce = launch_track_depth<gst::SPLIT_DK, 4>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
-    case GST_SPLIT_BEND_KICK_4: ce = launch_track_depth<gst::SPLIT_BK, 4>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
-    default: ce = launch_track_depth<gst::SPLIT_MK, 4>(romberg_depth, a, tab_bytes, seq_bytes, pair, st); break;
+    case GST_SPLIT_DRIFT_KICK: ce = launch_track_depth<gst::SPLIT_DK, 2>(romberg_depth, a, tab_bytes, seq_bytes, pair, st, chain); break;
+    case GST_SPLIT_BEND_KICK: ce = launch_track_depth<gst::SPLIT_BK, 2>(romberg_depth, a, tab_bytes, seq_bytes, pair, st, chain); break;
+    case GST_SPLIT_MATRIX_KICK: ce = launch_track_depth<gst::SPLIT_MK, 2>(romberg_depth, a, tab_bytes, seq_bytes, pair, st, chain); break;
+    case GST_SPLIT_DRIFT_KICK_4: ce = launch_track_depth<gst::SPLIT_DK, 4>(romberg_depth, a, tab_bytes, seq_bytes, pair, st, chain); break;
+    case GST_SPLIT_BEND_KICK_4: ce = launch_track_depth<gst::SPLIT_BK, 4>(romberg_depth, a, tab_bytes, seq_bytes, pair, st, chain); break;
+    default: ce = launch_track_depth<gst::SPLIT_MK, 4>(romberg_depth, a, tab_bytes, seq_bytes, pair, st, chain); break;
   }
   if (ce != cudaSuccess) return fail(GST_ECUDA, "track launch: %s", cudaGetErrorString(ce));
   // host-side bookkeeping of the reference energy: the same IEEE additions the kernel performs
@@ -484,7 +538,10 @@ static gst_status run_moments(gst_bunch* b, cudaStream_t st, bool second) {
   }
   CUDA_TRY(cudaGetLastError());
   CUDA_TRY(cudaMemcpyAsync(b->h_result, b->d_result, sizeof(double) * 2 * gst::RED_WIDTH, cudaMemcpyDeviceToHost, st));
+  int err = 0;
+  CUDA_TRY(cudaMemcpyAsync(&err, b->d_err, sizeof(int), cudaMemcpyDeviceToHost, st));
   CUDA_TRY(cudaStreamSynchronize(st));
+  if (err) return fail(GST_ECUDA, "track_chain_kernel: a chain handoff timed out (not every warp slot was resident)");
   return GST_OK;
 }
 

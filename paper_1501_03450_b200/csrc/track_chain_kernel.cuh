@@ -1,0 +1,120 @@
+// track_chain_kernel.cuh -- T1c: the fused tracking kernel with the bunch ROTATING over the warp slots of the chip.
+//
+// Why: a bunch of 65 536 particles is 2048 warps ("chains" of 32 particles) on 592 SM sub-partitions: 272 of
+// them hold 4 warps and 320 hold 3.  A sub-partition with 4 warps is saturated (profiles/r01_notes.md), so in
+// track_kernel.cuh the 3-warp ones finish after 77 % of the time and idle: 13 % of the chip's FP64 cycles.
+// Here the grid is exactly the 4 x 592 warp slots the chip holds; the turns are cut into chunks; in chunk k
+// chain c runs on slot (c + k * shift) mod slots, and the slots without a chain in that chunk wait.  The idle
+// slots wander over the chip, so every sub-partition carries the same load over the launch.  Nothing is
+// barrier-synchronised: a chain's chunk k may start as soon as its chunk k-1 is stored, which a per-chain flag
+// (release / acquire at GPU scope) announces; the state (72 B per particle) and the chain's reference energy
+// travel through global memory, bypassing the incoherent L1.
+//
+// Correct by induction on k (chunk 0 waits for nothing), provided every slot is resident: the host sizes the
+// grid with the occupancy API and falls back to track_kernel otherwise.  A bounded wait guards against a hang.
+// The arithmetic is the fused kernel's: results are bit-identical.
+#pragma once
+#include "track_kernel.cuh"
+
+namespace gst {
+
+struct ChainArgs {
+  int n_chains;        // ceil(n / 32)
+  int chunk_turns;     // turns per chunk
+  int shift;           // slots a chain moves per chunk
+  int* flag;           // [n_chains] chunks completed, zeroed before the launch
+  double* E0;          // [n_chains] reference energy after the chain's last chunk
+  int* err;            // set to 1 when a wait times out
+};
+
+__device__ __forceinline__ int ld_acquire(const int* p) {
+  int v;
+  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release(int* p, int v) {
+  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+template <int SPLIT, int DEPTH, int ORDER>
+__global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_chain_kernel(const TrackArgs a, const ChainArgs ch) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  DevElem* tab = reinterpret_cast<DevElem*>(smem_raw);
+  const uint32_t* seq = a.seq;
+  {
+    const int nw = a.n_unique * (int)(sizeof(DevElem) / sizeof(double));
+    const double* src = reinterpret_cast<const double*>(a.tab);
+    double* dst = reinterpret_cast<double*>(smem_raw);
+    for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
+    if (a.use_smem_seq) {
+      uint32_t* sseq = reinterpret_cast<uint32_t*>(smem_raw + (size_t)a.n_unique * sizeof(DevElem));
+      for (int i = threadIdx.x; i < a.n_seq; i += blockDim.x) sseq[i] = a.seq[i];
+      seq = sseq;
+    }
+    __syncthreads();
+  }
+  const int lane = threadIdx.x & 31;
+  const long long slots = (long long)gridDim.x * (TRACK_BLOCK / 32);
+  const long long slot = (long long)blockIdx.x * (TRACK_BLOCK / 32) + (threadIdx.x >> 5);
+  const long long n_chunks = (a.n_turns + ch.chunk_turns - 1) / ch.chunk_turns;
+  for (long long k = 0; k < n_chunks; ++k) {
+    long long c = (slot - k * ch.shift) % slots;
+    if (c < 0) c += slots;
+    if (c >= ch.n_chains) continue;                       // this slot has no chain in chunk k
+    if (k > 0) {                                          // chunk k-1 of this chain is stored
+      int tries = 0;
+      while (ld_acquire(ch.flag + c) < (int)k) {
+        __nanosleep(256);
+        if (++tries > (1 << 25)) { *ch.err = 1; return; }
+      }
+    }
+    const long long j = c * 32 + lane;
+    const bool valid = j < a.n && !__ldcg(a.lost + j);
+    State z;
+    z.X = z.Px = z.Y = z.Py = z.T = z.Pt = 0.0;
+    z.Sx = 0.0; z.Sy = 1.0; z.Ss = 0.0;
+    if (valid) {
+      z.X = __ldcg(a.p[0] + j); z.Px = __ldcg(a.p[1] + j); z.Y = __ldcg(a.p[2] + j); z.Py = __ldcg(a.p[3] + j);
+      z.T = __ldcg(a.p[4] + j); z.Pt = __ldcg(a.p[5] + j);
+      z.Sx = __ldcg(a.p[6] + j); z.Sy = __ldcg(a.p[7] + j); z.Ss = __ldcg(a.p[8] + j);
+    }
+    Ref ref;
+    ref_set(ref, k == 0 ? a.E0 : __ldcg(ch.E0 + c), a.mass);
+    PCon pc;
+    pcon_set(pc, z.Pt, ref, a.G);
+    bool lost = false;
+    typename SpinPolicy<DEPTH>::type spin(z);
+    const long long t0 = k * ch.chunk_turns;
+    const long long t1 = t0 + ch.chunk_turns < a.n_turns ? t0 + ch.chunk_turns : a.n_turns;
+    uint32_t nxt = seq[0];
+    for (long long turn = t0; turn < t1; ++turn) {
+#pragma unroll 1
+      for (int ie = 0; ie < a.n_seq; ++ie) {
+        const uint32_t cur = nxt;
+        nxt = seq[ie + 1 < a.n_seq ? ie + 1 : 0];
+        const DevElem& e = tab[cur >> 8];
+        const bool ok = element_step<SPLIT, ORDER>((int)(cur & 0xffu), z, e, pc, ref, a.G, spin);
+        if (!ok) {
+          lost = true;
+          z.X = z.Px = z.Y = z.Py = z.T = z.Pt = 0.0;
+          pcon_set(pc, 0.0, ref, a.G);
+        }
+      }
+    }
+    if (valid) {
+      if (lost) {
+        a.lost[j] = 1;
+      } else {
+        __stcg(a.p[0] + j, z.X); __stcg(a.p[1] + j, z.Px); __stcg(a.p[2] + j, z.Y); __stcg(a.p[3] + j, z.Py);
+        __stcg(a.p[4] + j, z.T); __stcg(a.p[5] + j, z.Pt);
+        __stcg(a.p[6] + j, z.Sx); __stcg(a.p[7] + j, z.Sy); __stcg(a.p[8] + j, z.Ss);
+      }
+    }
+    if (lane == 0) __stcg(ch.E0 + c, ref.E0);
+    __threadfence();
+    __syncwarp();
+    if (lane == 0) st_release(ch.flag + c, (int)k + 1);
+  }
+}
+
+}  // namespace gst

@@ -222,7 +222,7 @@ class Bunch:
             pass
 
 
-KERNEL_FUSED, KERNEL_PAIR = 0, 1
+KERNEL_FUSED, KERNEL_PAIR, KERNEL_FUSED_STATIC = 0, 1, 2
 
 
 def set_kernel_variant(variant):

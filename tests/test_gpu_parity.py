@@ -331,6 +331,28 @@ def test_pair_kernel_variant_is_bit_identical_to_the_fused_kernel(gst, split, de
         assert fused[4] == pair[4]
 
 
+def test_chain_rotation_is_bit_identical_to_the_static_launch(gst):
+    """65 553 particles fill the sub-partitions unevenly, so the default launch rotates the warps of particles
+    over the warp slots in chunks of turns (csrc/track_chain_kernel.cuh); state, lost flags and the ramping
+    reference energy must come out exactly as from the static launch."""
+    lat = mixed_lattice(ramp=True)
+    bm = W.beam(12.0)
+    n = 65536 + 17
+    st = W.gaussian_bunch(29, n, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
+    st[1, 5] = 1.5                                   # lost in the first chunk
+    st[3, 40000] = -2.0
+    rot = gpu_track(gst, lat, bm, st, 50, W.SPLIT_BEND_KICK, 4, 3)
+    try:
+        gst.set_kernel_variant(gst.KERNEL_FUSED_STATIC)
+        sta = gpu_track(gst, lat, bm, st, 50, W.SPLIT_BEND_KICK, 4, 3)
+    finally:
+        gst.set_kernel_variant(gst.KERNEL_FUSED)
+    assert np.array_equal(rot[1], sta[1]) and rot[1][5] and rot[1][40000]
+    keep = ~sta[1].astype(bool)
+    assert np.array_equal(rot[0][:, keep], sta[0][:, keep])
+    assert np.array_equal(rot[2], sta[2]) and rot[4] == sta[4]
+
+
 def test_chunked_tracking_is_bit_identical_to_one_call(gst):
     lat = mixed_lattice(ramp=True)
     bm = W.beam(12.0)
