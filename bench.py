@@ -273,7 +273,7 @@ def main():
     peak_meas, peak_ms = gst.fp64_peak()
     peak_rrr, _ = gst.fp64_peak_rrr()
     k_ms = float(np.mean(track_ms))
-    roof = {"bound": "alu", "unit": "TFLOP/s", "kernel": "gst::track_kernel<%d,%d>" % (split, depth),
+    roof = {"bound": "alu", "unit": "TFLOP/s", "kernel": "gst::%s<%d,%d,2>" % (bunch.last_kernel(), split, depth),
             "kernel_ms": k_ms, "peak": peak_meas, "peak_kind": "measured DFMA chains (gst_fp64_peak), this run",
             "peak_nominal": NOMINAL_FP64_TFLOPS,
             "peak_three_register_dfma": peak_rrr,   # context: DFMA R,R,R takes 3 cycles on B200
@@ -292,7 +292,8 @@ def main():
            "dtype": "f64", "data": "synthetic", "config": workload_config(cfg, n, turns, world),
            "particle_turns_per_s": float(n) * turns * world * args.steps / (total_ms * 1e-3),
            "polarization": [float(x) for x in pol], "wall_s": wall, "clocks": clocks, "e2e": e2e,
-           "gpu_launches": args.steps * 3, "launches_per_step": "track_kernel + moments_kernel + finalize_kernel",
+           "gpu_launches": args.steps * 3,
+           "launches_per_step": "%s + moments_kernel + finalize_kernel" % bunch.last_kernel(),
            "roofline": roof}
     if not args.no_cpu_baseline:
         out["cpu_baseline"] = cpu_baseline(cfg)

@@ -154,6 +154,10 @@ gst_status gst_polarization(gst_bunch* b, void* cuda_stream, double out[4], int6
 /* Geometric rms emittances (a13; reading A19), HOST out = {eps_x, eps_y}; synchronises the stream. */
 gst_status gst_emittance(gst_bunch* b, void* cuda_stream, double out_exy[2]);
 
+/* Name of the kernel the last gst_track / gst_track_pwc on this bunch launched: "track_kernel",
+ * "track_chain_kernel" or "track_pair_kernel" ("" before the first call).  Static storage.          */
+const char* gst_bunch_last_kernel(const gst_bunch* b);
+
 /* Copy the lost flags (1 = lost) to HOST memory, n bytes; synchronises the stream.                */
 gst_status gst_bunch_lost(gst_bunch* b, void* cuda_stream, uint8_t* host_out);
 

@@ -75,6 +75,7 @@ struct gst_bunch {
   int* d_chain_flag = nullptr;
   double* d_chain_E0 = nullptr;
   int* d_err = nullptr;
+  const char* last_kernel = "";
 };
 
 namespace {
@@ -212,14 +213,18 @@ SmemPlan plan_smem(size_t tab_bytes, size_t seq_bytes, size_t fixed, size_t budg
 
 // Does rotating the chains over the warp slots pay (track_chain_kernel.cuh)?  Only when the bunch fits the chip in
 // one wave but fills its sub-partitions unevenly, and there are enough turns to cut into chunks.
-bool chain_plan(long long n, long long n_turns, int slots, int sms, gst::ChainArgs* ch) {
+bool chain_plan(long long n, long long n_turns, long long steps_per_turn, int slots, int sms, gst::ChainArgs* ch) {
   const long long n_chains = (n + 31) / 32;
   const long long smsp = 4LL * sms;
   if (n_chains > slots || n_turns < 16 || 2 * n_chains < 3 * smsp) return false;
   const long long maxw = (n_chains + smsp - 1) / smsp;
   if ((double)maxw * smsp < 1.04 * (double)n_chains) return false;      // already even
   ch->n_chains = (int)n_chains;
-  ch->chunk_turns = (int)std::max<long long>(1, n_turns / 24);
+  // a chunk of ~16k particle-element-steps (a few ms per warp) is long against the handoff and short enough to mix:
+  // measured on config 3, 8 / 24 / 100 / 250 / 1000 chunks per 1000 turns give 1.56 / 1.63 / 1.65 / 1.67 / 1.67e11 steps/s
+  const long long want = (16384 + steps_per_turn - 1) / std::max<long long>(1, steps_per_turn);
+  ch->chunk_turns = (int)std::max<long long>(1, std::min<long long>(want, n_turns / 8));
+  // the idle band (slots - chains wide) moves by its own width: every slot idles once per slots/band chunks
   ch->shift = (slots - (int)n_chains) & ~1;
   return ch->shift > 0;
 }
@@ -264,10 +269,11 @@ cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, b
       if (e != cudaSuccess) return e;
       if (per_sm > gst::TRACK_MIN_BLOCKS) per_sm = gst::TRACK_MIN_BLOCKS;
       const int blocks = per_sm * sms;
-      if (chain_plan(a.n, a.n_turns, blocks * (gst::TRACK_BLOCK / 32), sms, chain)) {
+      if (chain_plan(a.n, a.n_turns, chain->n_chains /* steps per turn, set by the caller */, blocks * (gst::TRACK_BLOCK / 32), sms, chain)) {
         e = cudaMemsetAsync(chain->flag, 0, sizeof(int) * chain->n_chains, st);
         if (e != cudaSuccess) return e;
         ck<<<blocks, gst::TRACK_BLOCK, p.bytes, st>>>(a, *chain);
+        chain->n_chains = -chain->n_chains;     // tells the caller that the rotating launch was taken
         return cudaGetLastError();
       }
     }
@@ -439,6 +445,8 @@ gst_status gst_bunch_reference(const gst_bunch* b, double* gamma0, int64_t* turn
   return GST_OK;
 }
 
+const char* gst_bunch_last_kernel(const gst_bunch* b) { return b ? b->last_kernel : ""; }
+
 gst_status gst_bunch_set_reference(gst_bunch* b, const gst_beam* beam, int64_t turn) {
   if (!b || !beam || !(beam->gamma0 > 1.0) || !(beam->mass_eV > 0.0)) return fail(GST_EINVAL, "bad reference");
   b->E0 = beam->gamma0 * beam->mass_eV;
@@ -487,6 +495,7 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   chain_args.flag = b->d_chain_flag;
   chain_args.E0 = b->d_chain_E0;
   chain_args.err = b->d_err;
+  chain_args.n_chains = (int)std::min<int64_t>(gst_lattice_steps_per_turn(lat, table_slices), 1 << 30);   // in: steps per turn
   gst::ChainArgs* chain = g_variant.load() == GST_KERNEL_FUSED ? &chain_args : nullptr;
   a.use_smem_seq = 0;
   cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -500,6 +509,8 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
     default: ce = launch_track_depth<gst::SPLIT_MK, 4>(romberg_depth, a, tab_bytes, seq_bytes, pair, st, chain); break;
   }
   if (ce != cudaSuccess) return fail(GST_ECUDA, "track launch: %s", cudaGetErrorString(ce));
+  b->last_kernel = pair && romberg_depth >= 1 && (int)split < 3 ? "track_pair_kernel"
+                   : (chain && chain_args.n_chains < 0 ? "track_chain_kernel" : "track_kernel");
   // host-side bookkeeping of the reference energy: the same IEEE additions the kernel performs
   for (int64_t t = 0; t < n_turns; ++t)
     for (double dEs : lat->cav_dEs)

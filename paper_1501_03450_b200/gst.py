@@ -39,7 +39,7 @@ _dp = C.POINTER(C.c_double)
 EXPORTS = ["gst_lattice_create", "gst_lattice_destroy", "gst_lattice_steps_per_turn", "gst_bunch_init",
            "gst_bunch_destroy", "gst_track", "gst_polarization", "gst_emittance", "gst_bunch_lost",
            "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host", "gst_fp64_peak", "gst_selftest_math", "gst_last_error",
-           "gst_set_kernel_variant", "gst_fp64_peak_rrr", "gst_track_pwc"]
+           "gst_set_kernel_variant", "gst_fp64_peak_rrr", "gst_track_pwc", "gst_bunch_last_kernel"]
 
 
 def lib():
@@ -63,6 +63,8 @@ def lib():
         L.gst_track.argtypes = [vp, vp, C.c_int64, C.c_int, C.c_int, C.c_int, vp]
         L.gst_track_pwc.argtypes = [vp, vp, C.c_int64, C.c_int, C.c_int, C.c_int, vp]
         L.gst_track_pwc.restype = C.c_int
+        L.gst_bunch_last_kernel.argtypes = [vp]
+        L.gst_bunch_last_kernel.restype = C.c_char_p
         L.gst_polarization.argtypes = [vp, vp, _dp, C.POINTER(C.c_int64)]
         L.gst_emittance.argtypes = [vp, vp, _dp]
         L.gst_bunch_lost.argtypes = [vp, vp, C.POINTER(C.c_uint8)]
@@ -183,6 +185,9 @@ class Bunch:
         """gst_track_pwc; `order` is workloads.PWC_HALF_SLICE (0) or workloads.PWC_DKSKD (-1)."""
         _check(lib().gst_track_pwc(self._h, lattice._h, int(n_turns), int(split), int(n_slices),
                                    0 if int(order) == 0 else 1, self._stream(stream)))
+
+    def last_kernel(self):
+        return lib().gst_bunch_last_kernel(self._h).decode()
 
     def polarization(self, stream=None):
         out = (C.c_double * 4)()
