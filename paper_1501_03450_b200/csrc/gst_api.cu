@@ -270,11 +270,17 @@ cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, b
       if (per_sm > gst::TRACK_MIN_BLOCKS) per_sm = gst::TRACK_MIN_BLOCKS;
       const int blocks = per_sm * sms;
       if (chain_plan(a.n, a.n_turns, chain->n_chains /* steps per turn, set by the caller */, blocks * (gst::TRACK_BLOCK / 32), sms, chain)) {
-        e = cudaMemsetAsync(chain->flag, 0, sizeof(int) * chain->n_chains, st);
+        chain->n_sm = sms;
+        e = cudaMemsetAsync(chain->sm_scratch, 0, sizeof(int) * (chain->n_chains + 2 * gst::CHAIN_MAX_SMID + 1), st);
         if (e != cudaSuccess) return e;
-        ck<<<blocks, gst::TRACK_BLOCK, p.bytes, st>>>(a, *chain);
-        chain->n_chains = -chain->n_chains;     // tells the caller that the rotating launch was taken
-        return cudaGetLastError();
+        // a cooperative launch guarantees what the hand-offs rely on: every block of the grid is resident
+        void* kargs[2] = {(void*)&a, (void*)chain};
+        e = cudaLaunchCooperativeKernel((const void*)ck, dim3(blocks), dim3(gst::TRACK_BLOCK), kargs, p.bytes, st);
+        if (e == cudaSuccess) {
+          chain->n_chains = -chain->n_chains;   // tells the caller that the rotating launch was taken
+          return cudaSuccess;
+        }
+        (void)cudaGetLastError();               // e.g. cudaErrorCooperativeLaunchTooLarge: take the static launch
       }
     }
   }
@@ -413,7 +419,8 @@ gst_status gst_bunch_init(double* x, double* px, double* y, double* py, double* 
   if (ce == cudaSuccess) ce = cudaMalloc(&b->d_result, sizeof(double) * 2 * gst::RED_WIDTH);
   if (ce == cudaSuccess) ce = cudaMallocHost(&b->h_result, sizeof(double) * 2 * gst::RED_WIDTH);
   const size_t n_chains = (n + 31) / 32 + 1;
-  if (ce == cudaSuccess) ce = cudaMalloc(&b->d_chain_flag, sizeof(int) * n_chains);
+  // [sm scratch | chain flags], zeroed together before every rotating launch
+  if (ce == cudaSuccess) ce = cudaMalloc(&b->d_chain_flag, sizeof(int) * (n_chains + 2 * gst::CHAIN_MAX_SMID + 1));
   if (ce == cudaSuccess) ce = cudaMalloc(&b->d_chain_E0, sizeof(double) * n_chains);
   if (ce == cudaSuccess) ce = cudaMalloc(&b->d_err, sizeof(int));
   if (ce == cudaSuccess) ce = cudaMemset(b->d_err, 0, sizeof(int));
@@ -492,7 +499,8 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   if (tab_bytes > 24 * 1024) return fail(GST_EINVAL, "too many unique elements for the shared-memory table (%zu)", lat->uniq.size());
   const bool pair = g_variant.load() == GST_KERNEL_PAIR;
   gst::ChainArgs chain_args;
-  chain_args.flag = b->d_chain_flag;
+  chain_args.sm_scratch = b->d_chain_flag;
+  chain_args.flag = b->d_chain_flag + 2 * gst::CHAIN_MAX_SMID + 1;
   chain_args.E0 = b->d_chain_E0;
   chain_args.err = b->d_err;
   chain_args.n_chains = (int)std::min<int64_t>(gst_lattice_steps_per_turn(lat, table_slices), 1 << 30);   // in: steps per turn
