@@ -110,10 +110,11 @@ def cpu_baseline(cfg, budget_s=15.0):
     spt = W.steps_per_turn(lat, cfg["n_slices"])
     n = min(cfg["state"].shape[1], cores * 16)
     st = cfg["state"][:, :n]
+    O.track(lat, beam, st, 1, cfg["split"], cfg["n_slices"], cfg["depth"], prec=O.PREC_DOUBLE, threads=cores)   # warm: library load, threads
     t0 = time.perf_counter()
-    O.track(lat, beam, st, 1, cfg["split"], cfg["n_slices"], cfg["depth"], prec=O.PREC_DOUBLE, threads=cores)
-    t1 = time.perf_counter() - t0
-    turns = int(max(2, min(20000, budget_s / max(t1, 1e-3))))
+    O.track(lat, beam, st, 8, cfg["split"], cfg["n_slices"], cfg["depth"], prec=O.PREC_DOUBLE, threads=cores)
+    t1 = (time.perf_counter() - t0) / 8
+    turns = int(max(2, min(20000, budget_s / max(t1, 1e-4))))
     t0 = time.perf_counter()
     O.track(lat, beam, st, turns, cfg["split"], cfg["n_slices"], cfg["depth"], prec=O.PREC_DOUBLE, threads=cores)
     dt = time.perf_counter() - t0
