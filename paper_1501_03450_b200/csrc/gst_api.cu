@@ -213,6 +213,13 @@ SmemPlan plan_smem(size_t tab_bytes, size_t seq_bytes, size_t fixed, size_t budg
 
 // Does rotating the chains over the warp slots pay (track_chain_kernel.cuh)?  Only when the bunch fits the chip in
 // one wave but fills its sub-partitions unevenly, and there are enough turns to cut into chunks.
+// host-side request for the rotating launch: device arguments, what the planner needs, and whether it was taken
+struct ChainLaunch {
+  gst::ChainArgs args;
+  long long steps_per_turn = 1;
+  bool taken = false;
+};
+
 bool chain_plan(long long n, long long n_turns, long long steps_per_turn, int slots, int sms, gst::ChainArgs* ch) {
   const long long n_chains = (n + 31) / 32;
   const long long smsp = 4LL * sms;
@@ -231,7 +238,7 @@ bool chain_plan(long long n, long long n_turns, long long steps_per_turn, int sl
 
 template <int SPLIT, int DEPTH, int ORDER>
 cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, bool pair, cudaStream_t st,
-                         gst::ChainArgs* chain = nullptr) {
+                         ChainLaunch* chain = nullptr) {
   if constexpr (ORDER == 2 && DEPTH >= 1) {   // the experimental pair kernel: second-order maps, edge scheme only
   if (pair) {
     // T1p: two threads per particle.  Shared memory per block is budgeted so that MIN_BLOCKS blocks stay
@@ -269,15 +276,16 @@ cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, b
       if (e != cudaSuccess) return e;
       if (per_sm > gst::TRACK_MIN_BLOCKS) per_sm = gst::TRACK_MIN_BLOCKS;
       const int blocks = per_sm * sms;
-      if (chain_plan(a.n, a.n_turns, chain->n_chains /* steps per turn, set by the caller */, blocks * (gst::TRACK_BLOCK / 32), sms, chain)) {
-        chain->n_sm = sms;
-        e = cudaMemsetAsync(chain->sm_scratch, 0, sizeof(int) * (chain->n_chains + 2 * gst::CHAIN_MAX_SMID + 1), st);
+      gst::ChainArgs& ca = chain->args;
+      if (chain_plan(a.n, a.n_turns, chain->steps_per_turn, blocks * (gst::TRACK_BLOCK / 32), sms, &ca)) {
+        ca.n_sm = sms;
+        e = cudaMemsetAsync(ca.sm_scratch, 0, sizeof(int) * (ca.n_chains + 2 * gst::CHAIN_MAX_SMID + 1), st);
         if (e != cudaSuccess) return e;
         // a cooperative launch guarantees what the hand-offs rely on: every block of the grid is resident
-        void* kargs[2] = {(void*)&a, (void*)chain};
+        void* kargs[2] = {(void*)&a, (void*)&ca};
         e = cudaLaunchCooperativeKernel((const void*)ck, dim3(blocks), dim3(gst::TRACK_BLOCK), kargs, p.bytes, st);
         if (e == cudaSuccess) {
-          chain->n_chains = -chain->n_chains;   // tells the caller that the rotating launch was taken
+          chain->taken = true;
           return cudaSuccess;
         }
         (void)cudaGetLastError();               // e.g. cudaErrorCooperativeLaunchTooLarge: take the static launch
@@ -297,7 +305,7 @@ cudaError_t launch_track(gst::TrackArgs a, size_t tab_bytes, size_t seq_bytes, b
 
 template <int SPLIT, int ORDER>
 cudaError_t launch_track_depth(int depth, const gst::TrackArgs& a, size_t tb, size_t sb, bool pair, cudaStream_t st,
-                               gst::ChainArgs* chain) {
+                               ChainLaunch* chain) {
   if (ORDER == 2 && depth == 0) return launch_track<SPLIT, 0, 2>(a, tb, sb, false, st);
   if (ORDER == 2 && depth == -1) return launch_track<SPLIT, -1, 2>(a, tb, sb, false, st);
   switch (depth) {
@@ -498,13 +506,13 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   size_t seq_bytes = (lat->seq.size() * sizeof(uint32_t) + 15) & ~size_t(15);
   if (tab_bytes > 24 * 1024) return fail(GST_EINVAL, "too many unique elements for the shared-memory table (%zu)", lat->uniq.size());
   const bool pair = g_variant.load() == GST_KERNEL_PAIR;
-  gst::ChainArgs chain_args;
-  chain_args.sm_scratch = b->d_chain_flag;
-  chain_args.flag = b->d_chain_flag + 2 * gst::CHAIN_MAX_SMID + 1;
-  chain_args.E0 = b->d_chain_E0;
-  chain_args.err = b->d_err;
-  chain_args.n_chains = (int)std::min<int64_t>(gst_lattice_steps_per_turn(lat, table_slices), 1 << 30);   // in: steps per turn
-  gst::ChainArgs* chain = g_variant.load() == GST_KERNEL_FUSED ? &chain_args : nullptr;
+  ChainLaunch chain_req;
+  chain_req.args.sm_scratch = b->d_chain_flag;
+  chain_req.args.flag = b->d_chain_flag + 2 * gst::CHAIN_MAX_SMID + 1;
+  chain_req.args.E0 = b->d_chain_E0;
+  chain_req.args.err = b->d_err;
+  chain_req.steps_per_turn = gst_lattice_steps_per_turn(lat, table_slices);
+  ChainLaunch* chain = g_variant.load() == GST_KERNEL_FUSED ? &chain_req : nullptr;
   a.use_smem_seq = 0;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   cudaError_t ce;
@@ -518,7 +526,7 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   }
   if (ce != cudaSuccess) return fail(GST_ECUDA, "track launch: %s", cudaGetErrorString(ce));
   b->last_kernel = pair && romberg_depth >= 1 && (int)split < 3 ? "track_pair_kernel"
-                   : (chain && chain_args.n_chains < 0 ? "track_chain_kernel" : "track_kernel");
+                   : (chain_req.taken ? "track_chain_kernel" : "track_kernel");
   // host-side bookkeeping of the reference energy: the same IEEE additions the kernel performs
   for (int64_t t = 0; t < n_turns; ++t)
     for (double dEs : lat->cav_dEs)

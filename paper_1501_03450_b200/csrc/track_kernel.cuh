@@ -1073,7 +1073,10 @@ __device__ __forceinline__ bool element_step(int type, State& z, const DevElem& 
 // fit per sub-partition (888 slots) and the last 136 blocks run alone in a second wave (measured:
 // 85 ms vs 53 ms per 20 turns, profiles/r01_notes.md).
 constexpr int TRACK_BLOCK = 64;
-constexpr int TRACK_MIN_BLOCKS = 8;
+#ifndef GST_TRACK_MIN_BLOCKS
+#define GST_TRACK_MIN_BLOCKS 8
+#endif
+constexpr int TRACK_MIN_BLOCKS = GST_TRACK_MIN_BLOCKS;
 
 template <int SPLIT, int DEPTH, int ORDER>
 __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_kernel(const TrackArgs a) {
