@@ -353,6 +353,23 @@ def test_chain_rotation_is_bit_identical_to_the_static_launch(gst):
     assert np.array_equal(rot[2], sta[2]) and rot[4] == sta[4]
 
 
+@pytest.mark.parametrize("n,turns", [(28449, 16), (47360, 17), (75712, 33), (75744, 16), (65536, 40)])
+def test_chain_rotation_edge_sizes(gst, n, turns):
+    """Rotating launch at the edges of its plan: 1.5 warps per sub-partition, a shift of 2 slots, one chain short
+    of a full chip (no rotation possible), chunk counts that do not divide the turns."""
+    lat = mixed_lattice(ramp=True)
+    bm = W.beam(12.0)
+    st = W.gaussian_bunch(31, n, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
+    rot = gpu_track(gst, lat, bm, st, turns, W.SPLIT_MATRIX_KICK, 2, 2)
+    try:
+        gst.set_kernel_variant(gst.KERNEL_FUSED_STATIC)
+        sta = gpu_track(gst, lat, bm, st, turns, W.SPLIT_MATRIX_KICK, 2, 2)
+    finally:
+        gst.set_kernel_variant(gst.KERNEL_FUSED)
+    assert not sta[1].any() and np.array_equal(rot[1], sta[1])
+    assert np.array_equal(rot[0], sta[0]) and rot[4] == sta[4]
+
+
 def test_chunked_tracking_is_bit_identical_to_one_call(gst):
     lat = mixed_lattice(ramp=True)
     bm = W.beam(12.0)
