@@ -223,7 +223,7 @@ struct ChainLaunch {
 bool chain_plan(long long n, long long n_turns, long long steps_per_turn, int slots, int sms, gst::ChainArgs* ch) {
   const long long n_chains = (n + 31) / 32;
   const long long smsp = 4LL * sms;
-  if (n_chains > slots || n_turns < 16 || 2 * n_chains < 3 * smsp) return false;
+  if (n_chains > slots || n_turns < 16 || n_chains < 2 * smsp) return false;   // below 2 warps per sub-partition the static launch wins (measured)
   const long long maxw = (n_chains + smsp - 1) / smsp;
   if ((double)maxw * smsp < 1.04 * (double)n_chains) return false;      // already even
   ch->n_chains = (int)n_chains;

@@ -353,9 +353,9 @@ def test_chain_rotation_is_bit_identical_to_the_static_launch(gst):
     assert np.array_equal(rot[2], sta[2]) and rot[4] == sta[4]
 
 
-@pytest.mark.parametrize("n,turns", [(28449, 16), (47360, 17), (75712, 33), (75744, 16), (65536, 40)])
+@pytest.mark.parametrize("n,turns", [(37920, 16), (47360, 17), (75712, 33), (75744, 16), (65536, 40)])
 def test_chain_rotation_edge_sizes(gst, n, turns):
-    """Rotating launch at the edges of its plan: 1.5 warps per sub-partition, a shift of 2 slots, one chain short
+    """Rotating launch at the edges of its plan: just over 2 warps per sub-partition, a shift of 2 slots, one chain short
     of a full chip (no rotation possible), chunk counts that do not divide the turns."""
     lat = mixed_lattice(ramp=True)
     bm = W.beam(12.0)
