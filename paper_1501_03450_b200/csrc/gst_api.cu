@@ -211,8 +211,10 @@ SmemPlan plan_smem(size_t tab_bytes, size_t seq_bytes, size_t fixed, size_t budg
   return p;
 }
 
-// Does rotating the chains over the warp slots pay (track_chain_kernel.cuh)?  Only when the bunch fits the chip in
-// one wave but fills its sub-partitions unevenly, and there are enough turns to cut into chunks.
+// Does laying the (chain, chunk) work items over the warp slots pay (track_chain_kernel.cuh)?  When a plain launch
+// would leave sub-partitions unevenly filled within one wave (by more than 4 %) or would need a small second wave,
+// the bunch averages at least 2 warps per sub-partition (below that the static launch measured 2-5 % faster) and
+// there are enough turns to cut into chunks.
 // host-side request for the rotating launch: device arguments, what the planner needs, and whether it was taken
 struct ChainLaunch {
   gst::ChainArgs args;
@@ -223,17 +225,23 @@ struct ChainLaunch {
 bool chain_plan(long long n, long long n_turns, long long steps_per_turn, int slots, int sms, gst::ChainArgs* ch) {
   const long long n_chains = (n + 31) / 32;
   const long long smsp = 4LL * sms;
-  if (n_chains > slots || n_turns < 16 || n_chains < 2 * smsp) return false;   // below 2 warps per sub-partition the static launch wins (measured)
-  const long long maxw = (n_chains + smsp - 1) / smsp;
-  if ((double)maxw * smsp < 1.04 * (double)n_chains) return false;      // already even
+  if (n_turns < 16 || n_chains < 2 * smsp || n_chains % slots == 0) return false;
+  if (n_chains <= slots) {
+    // one wave: does the plain launch fill the sub-partitions evenly (within 4 %)?
+    const long long maxw = (n_chains + smsp - 1) / smsp;
+    if ((double)n_chains > 0.96 * (double)(maxw * smsp)) return false;
+  } else if (2 * n_chains >= 3 * slots) {
+    // one and a half waves or more: the plain launch refills the SMs block by block and its thin last wave runs
+    // fast; measured (config 3, 100 turns) 131 072 / 200 000 / 262 144 particles: plain 1.67 / 1.67 / 1.73e11
+    // against 1.63 / 1.65 / 1.65e11 for the sequence; 80 000 / 100 000: plain 1.34 / 1.47e11 against 1.65 / 1.64e11
+    return false;
+  }
   ch->n_chains = (int)n_chains;
   // a chunk of ~16k particle-element-steps (a few ms per warp) is long against the handoff and short enough to mix:
   // measured on config 3, 8 / 24 / 100 / 250 / 1000 chunks per 1000 turns give 1.56 / 1.63 / 1.65 / 1.67 / 1.67e11 steps/s
   const long long want = (16384 + steps_per_turn - 1) / std::max<long long>(1, steps_per_turn);
   ch->chunk_turns = (int)std::max<long long>(1, std::min<long long>(want, n_turns / 8));
-  // the idle band (slots - chains wide) moves by its own width: every slot idles once per slots/band chunks
-  ch->shift = (slots - (int)n_chains) & ~1;
-  return ch->shift > 0;
+  return true;
 }
 
 template <int SPLIT, int DEPTH, int ORDER>

@@ -2,21 +2,27 @@
 //
 // Why: a bunch of 65 536 particles is 2048 warps ("chains" of 32 particles) on 592 SM sub-partitions: 272 of
 // them hold 4 warps and 320 hold 3.  A sub-partition with 4 warps is saturated (profiles/r01_notes.md), so in
-// track_kernel.cuh the 3-warp ones finish after 77 % of the time and idle: 13 % of the chip's FP64 cycles.
-// Here the grid is exactly the 4 x 592 warp slots the chip holds; the turns are cut into chunks; in chunk k
-// chain c runs on slot (c + k * shift) mod slots, and the slots without a chain in that chunk wait.  The idle
-// slots wander over the chip, so every sub-partition carries the same load over the launch.  Nothing is
-// barrier-synchronised: a chain's chunk k may start as soon as its chunk k-1 is stored, which a per-chain flag
-// (release / acquire at GPU scope) announces; the state (72 B per particle) and the chain's reference energy
-// travel through global memory, bypassing the incoherent L1.
+// track_kernel.cuh the 3-warp ones finish after 77 % of the time and idle: 13 % of the chip's FP64 cycles.  A
+// bunch of 262 144 particles is 3.46 WAVES of blocks, and the last wave leaves half the chip empty.
+// Here the grid is exactly the S = 4 x 592 warp slots the chip holds, the turns are cut into chunks, and the
+// work items (chain c, chunk k) are laid out in one sequence  p = k * M + c  (M chains): slot v takes the
+// positions p = v, v + S, v + 2S, ...  Consecutive chunks of a chain are M positions apart, so
+//   M > S : every slot is busy all the time and a chain rests in global memory between its chunks -- no waves;
+//   M < S : in every round S - M slots find that their chain's previous chunk is still being computed and
+//           wait; because S is not a multiple of M these idle slots wander over the chip, so every
+//           sub-partition carries the same load over the launch.
+// Nothing is barrier-synchronised: chunk k of a chain may start as soon as its chunk k-1 is stored, which a
+// per-chain flag (release / acquire at GPU scope) announces; the state (72 B per particle) and the chain's
+// reference energy travel through global memory, bypassing the incoherent L1.
 //
 // Which slots idle together matters: the slots are numbered v = (warp index on its SM) * n_sm + (rank of the SM), from
-// %smid and two atomics at kernel start, so that the band of idle slots [n_chains, slots) -- consecutive in v,
-// moved by its own width every chunk -- is always spread evenly over ALL SMs, whatever order the hardware
-// places the blocks in (with the block index as slot number a cooperative launch was 4 % slower than a plain one).
+// %smid and two atomics at kernel start, so that slots that are neighbours in v -- the ones that idle together -- sit
+// on different SMs, whatever order the hardware places the blocks in (with the block index as slot number a
+// cooperative launch was 4 % slower than a plain one).
 //
-// Correct by induction on k (chunk 0 waits for nothing), provided every slot is resident: the host sizes the
-// grid with the occupancy API and falls back to track_kernel otherwise.  A bounded wait guards against a hang.
+// Correct by induction on p (a position waits only for position p - M, which its slot reaches earlier in its own
+// order), provided every slot is resident: the host launches the occupancy-sized grid cooperatively and falls
+// back to track_kernel otherwise.  Bounded waits guard against a hang.
 // The arithmetic is the fused kernel's: results are bit-identical.
 #pragma once
 #include "track_kernel.cuh"
@@ -26,7 +32,6 @@ namespace gst {
 struct ChainArgs {
   int n_chains;        // ceil(n / 32)
   int chunk_turns;     // turns per chunk
-  int shift;           // slots a chain moves per chunk
   int n_sm;            // SMs in use = gridDim.x / blocks per SM
   int* sm_scratch;     // [2 * CHAIN_MAX_SMID + 1] blocks arrived per SM, rank + 1 per SM, SMs ranked; zeroed with flag[]
   int* flag;           // [n_chains] chunks completed, zeroed before the launch
@@ -92,10 +97,10 @@ __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_chain_ker
   }
   const long long slot = (long long)(s_local * (TRACK_BLOCK / 32) + (threadIdx.x >> 5)) * ch.n_sm + s_rank;
   const long long n_chunks = (a.n_turns + ch.chunk_turns - 1) / ch.chunk_turns;
-  for (long long k = 0; k < n_chunks; ++k) {
-    long long c = (slot - k * ch.shift) % slots;
-    if (c < 0) c += slots;
-    if (c >= ch.n_chains) continue;                       // this slot has no chain in chunk k
+  const long long M = ch.n_chains;
+  const long long total = n_chunks * M;
+  for (long long p = slot; p < total; p += slots) {
+    const long long k = p / M, c = p - k * M;             // chunk k of chain c
     if (k > 0) {                                          // chunk k-1 of this chain is stored
       int tries = 0;
       while (ld_acquire(ch.flag + c) < (int)k) {

@@ -353,10 +353,11 @@ def test_chain_rotation_is_bit_identical_to_the_static_launch(gst):
     assert np.array_equal(rot[2], sta[2]) and rot[4] == sta[4]
 
 
-@pytest.mark.parametrize("n,turns", [(37920, 16), (47360, 17), (75712, 33), (75744, 16), (65536, 40)])
+@pytest.mark.parametrize("n,turns", [(37920, 16), (47360, 17), (75712, 33), (75744, 16), (65536, 40), (80000, 17),
+                                     (262144 + 5, 16)])
 def test_chain_rotation_edge_sizes(gst, n, turns):
     """Rotating launch at the edges of its plan: just over 2 warps per sub-partition, a shift of 2 slots, one chain short
-    of a full chip (no rotation possible), chunk counts that do not divide the turns."""
+    of a full chip, chunk counts that do not divide the turns, more chains than warp slots (1.06 and 3.46 waves)."""
     lat = mixed_lattice(ramp=True)
     bm = W.beam(12.0)
     st = W.gaussian_bunch(31, n, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
