@@ -1073,13 +1073,14 @@ __device__ __forceinline__ bool element_step(int type, State& z, const DevElem& 
 // fit per sub-partition (888 slots) and the last 136 blocks run alone in a second wave (measured:
 // 85 ms vs 53 ms per 20 turns, profiles/r01_notes.md).
 constexpr int TRACK_BLOCK = 64;
-#ifndef GST_TRACK_MIN_BLOCKS
-#define GST_TRACK_MIN_BLOCKS 8
-#endif
-constexpr int TRACK_MIN_BLOCKS = GST_TRACK_MIN_BLOCKS;
+constexpr int TRACK_MIN_BLOCKS = 8;
+// The fourth-order matrix-kick map carries two tables of linear-flow coefficients: at 128 registers it spills
+// 800 B per thread.  With 6 blocks per SM (3 warps per sub-partition, 167 registers, no spills) it measured 20 %
+// faster; every other instantiation is equal or slightly slower that way (profiles/r01_notes.md).
+__host__ __device__ constexpr int track_min_blocks(int split, int order) { return (split == SPLIT_MK && order == 4) ? 6 : TRACK_MIN_BLOCKS; }
 
 template <int SPLIT, int DEPTH, int ORDER>
-__global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_kernel(const TrackArgs a) {
+__global__ void __launch_bounds__(TRACK_BLOCK, track_min_blocks(SPLIT, ORDER)) track_kernel(const TrackArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   DevElem* tab = reinterpret_cast<DevElem*>(smem_raw);
   const uint32_t* seq = a.seq;
