@@ -126,6 +126,11 @@ struct PCon {
   double tA;    // 2 Pt/(beta0 gamma0)^2 + Pt^2/beta0   (time-of-flight numerator, see drift())
   double tq;    // 1/beta0 - (1/beta0 + Pt)/P, cancellation-free
   double ibpt;  // 1/beta0 + Pt
+  // The last drift's 1/Ps and time-of-flight factor.  A drift changes no momentum, so a drift that directly
+  // follows a drift (long straights are cut into pieces) reuses them instead of two MUFU + Newton chains:
+  // the same numbers, three FMAs.  Cleared by every element that can change Px, Py or Pt.
+  double d_iPs, d_num;
+  bool d_valid;
 };
 
 __device__ __forceinline__ void ref_set(Ref& r, double E0, double mass) {
@@ -149,6 +154,7 @@ __device__ __forceinline__ void pcon_set(PCon& c, double Pt, const Ref& r, doubl
   // (P-1)/beta0 - Pt = [tA - Pt (P-1)]/(P+1),  P-1 = e0/(P+1)
   double ip1 = 1.0 / (c.P + 1.0);
   c.tq = (c.tA - Pt * c.e0 * ip1) * ip1 * c.iP;
+  c.d_valid = false;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -313,19 +319,24 @@ struct State {
 
 // a3: exact drift (29b).  T' = 1/beta0 - (1/beta0+Pt)/Ps is evaluated as
 // [(Ps-1)/beta0 - Pt]/Ps with Ps-1 = (Ps^2-1)/(Ps+1) and the O(Pt) terms combined analytically.
-__device__ __forceinline__ bool drift(State& z, double L, const PCon& c, const Ref& r) {
-  double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
-  double ps2m1 = c.e0 - pt2;
-  double ps2 = 1.0 + ps2m1;
-  double iPs = rsqrt_nr(ps2);
-  double Ps = ps2 * iPs;
-  double iPs1 = rcp_nr(Ps + 1.0);
-  double LiPs = L * iPs;
+__device__ __forceinline__ bool drift(State& z, double L, PCon& c, const Ref& r) {
+  if (!c.d_valid) {
+    double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
+    double ps2m1 = c.e0 - pt2;
+    double ps2 = 1.0 + ps2m1;
+    double iPs = rsqrt_nr(ps2);
+    double Ps = ps2 * iPs;
+    double iPs1 = rcp_nr(Ps + 1.0);
+    c.d_iPs = iPs;
+    c.d_num = (fma(-pt2, r.ibeta0, c.tA) - z.Pt * ps2m1 * iPs1) * iPs1;
+    c.d_valid = ps2 > 0.0;
+    if (!c.d_valid) return false;
+  }
+  const double LiPs = L * c.d_iPs;
   z.X = fma(LiPs, z.Px, z.X);
   z.Y = fma(LiPs, z.Py, z.Y);
-  double num = (fma(-pt2, r.ibeta0, c.tA) - z.Pt * ps2m1 * iPs1) * iPs1;
-  z.T = fma(LiPs, num, z.T);
-  return ps2 > 0.0;
+  z.T = fma(LiPs, c.d_num, z.T);
+  return true;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -1010,6 +1021,7 @@ __constant__ double FRINGE_INV_M[4] = {1.0 / 2.0, 1.0 / 3.0, 1.0 / 4.0, 1.0 / 5.
 template <int SPLIT, int ORDER, class Spin>
 __device__ __forceinline__ bool element_step(int type, State& z, const DevElem& e, PCon& pc, Ref& ref, double G, Spin& spin) {
   if (type == K_DRIFT) return drift(z, e.L, pc, ref);
+  if (type != K_MARKER && type != K_SNAKE) pc.d_valid = false;     // the momenta may change: the cached drift factors expire
   if (type == K_QUAD) {
     if (SPLIT == SPLIT_MK) return quad_mk<ORDER>(z, e, pc, spin);
     return mult_dk<ORDER>(z, e, pc, ref, spin);
