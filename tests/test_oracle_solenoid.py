@@ -12,6 +12,7 @@ kick (40)  (section 3.7, section 4.4).
 The paper's solenoid (1.3 T, 2.1 m) and its 1.2 GeV proton are the test case.
 """
 import math
+import os
 
 import numpy as np
 import pytest
@@ -22,13 +23,18 @@ from paper_1501_03450_b200 import workloads as W
 from test_oracle_orbit import S_SYMP
 from test_oracle_spin import _tbmt_axis
 
+GLD = {}
+for _line in open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "paper_solenoid_inputs.txt")):
+    _f = _line.split("#")[0].split()
+    if len(_f) == 2:
+        GLD[_f[0]] = float(_f[1])
 MASS = W.MASS_PROTON_EV
-EKIN = 1.2e9                                        # P:729 "1.2 GeV proton" (kinetic energy reading, DESIGN R9)
+EKIN = GLD["proton_GeV"] * 1e9                      # P:729 "1.2 GeV proton" (kinetic energy reading, DESIGN R9)
 GAMMA = 1.0 + EKIN / MASS
 BETA = math.sqrt(1.0 - 1.0 / GAMMA ** 2)
 BRHO = MASS * GAMMA * BETA / 299792458.0            # T m
-KS = 1.3 / BRHO                                     # b_0/(B rho)_o for the 1.3 T solenoid
-LSOL = 2.1
+KS = GLD["solenoid_B_T"] / BRHO                     # b_0/(B rho)_o for the 1.3 T solenoid
+LSOL = GLD["solenoid_L_m"]
 BEAM = W.beam(GAMMA)
 G = BEAM["G"]
 Z0 = np.array([1.2e-2, 2.0e-3, -0.9e-2, -1.5e-3, 0.0, 1.5e-3])
