@@ -2,6 +2,7 @@
 
     python -m paper_1501_03450_b200.studies ramp  [--particles N] [--turns T] [--chunk 100] [--out FILE.md]
     python -m paper_1501_03450_b200.studies sweep [--particles N] [--turns T] [--out FILE.md]
+    python -m paper_1501_03450_b200.studies fig7  [--out FILE.md]
 
 ramp  : BASELINE configs[3] (SURVEY config 4): the RHIC-like ring with its cavity ramping the energy by
         100 keV/turn from G*gamma = 45.0, 2^20 particles, 5000 turns; the bunch polarization, emittances
@@ -12,6 +13,11 @@ sweep : BASELINE configs[4] (SURVEY config 5): accuracy vs throughput on the rin
         Errors are the paper's (44) P:622 and (46) P:733 against a reference by refinement, as the paper
         does: matrix-kick, 128 slices, depth 6 -- computed by the same library; that this
         reference equals the CPU oracle's is what tests/test_gpu_parity.py::test_config5_reference_run checks.
+
+fig7  : the paper's single-element study (Fig. 7): spin error of its test particle (footnote 5)
+        across the RHIC IR quadrupole (1.83 m, 70 T/m), arc dipole (9.45 m, 2.225 deg) and the 1.3 T,
+        2.1 m solenoid at 200 GeV and at 1.2 GeV, against the number of slices, for mid-slice PWC
+        and for k = 0..3 Romberg iterations on the edge scheme; reference = 256 slices, k = 3.
 
 Every number of the hot path comes from the CUDA kernels; torch is used for device memory, the error
 norms of the report and nothing else.  One JSON line per report row on stdout; --out adds a markdown table.
@@ -141,6 +147,66 @@ def sweep(args):
     lat.close()
 
 
+def fig7(args):
+    """Inputs are the ones the paper prints (cited above); the element maps are matrix-kick / exact."""
+    import math
+    import torch
+    from . import gst
+    mp_gev = W.MASS_PROTON_EV / 1e9
+
+    def brho(gamma):
+        return W.MASS_PROTON_EV * gamma * W.beta_of_gamma(gamma) / 299792458.0
+
+    g200 = 200.0 / mp_gev                                    # "200 GeV protons": total energy (DESIGN R3)
+    g12 = 1.0 + 1.2 / mp_gev                                 # "1.2 GeV proton": kinetic energy (DESIGN R9)
+    cases = [("IR quadrupole 1.83 m, 70 T/m, 200 GeV", W.quad(1.83, 70.0 / brho(g200)), g200),
+             ("arc dipole 9.45 m, 2.225 deg, 200 GeV", W.sbend(9.45, math.radians(2.225)), g200),
+             ("solenoid 2.1 m, 1.3 T, 200 GeV", W.solenoid(2.1, 1.3 / brho(g200)), g200),
+             ("solenoid 2.1 m, 1.3 T, 1.2 GeV", W.solenoid(2.1, 1.3 / brho(g12)), g12)]
+    slices = [1, 2, 4, 8, 16, 32, 64, 128]
+    lines = []
+    for name, elem, gamma in cases:
+        b0 = W.beta_of_gamma(gamma)
+        delta = 1e-3
+        pt = math.sqrt(1.0 / b0 ** 2 + 2 * delta + delta ** 2) - 1.0 / b0     # A22
+        s0 = np.array([2.0, 10.0, 1.0]) / math.sqrt(105.0)                    # (0.1952, 0.9759, 0.0976), P:654
+        st = np.zeros((9, 32))
+        st[:, :] = np.array([1.0e-3, 0.1e-3, 0.0, -0.2e-3, 0.0, pt, s0[0], s0[1], s0[2]])[:, None]
+        lat = gst.Lattice(W.lattice([elem]), W.beam(gamma))
+
+        def spin(n, depth):
+            dev = _device_state(torch, st)
+            b = gst.Bunch(dev)
+            if depth >= 1:
+                b.track(lat, 1, W.SPLIT_MATRIX_KICK, n, depth)
+            else:
+                b.track_pwc(lat, 1, W.SPLIT_MATRIX_KICK, n, W.PWC_HALF_SLICE)
+            out = dev[6:9, 0].cpu().numpy()
+            b.close()
+            return out
+        ref = spin(256, 4)
+        rows = []
+        for n in slices:
+            errs = {"pwc": float(np.linalg.norm(spin(n, 0) - ref))}
+            for d in (1, 2, 3, 4):
+                errs["k%d" % (d - 1)] = float(np.linalg.norm(spin(n, d) - ref)) if n % (1 << (d - 1)) == 0 else None
+            rows.append((n, errs))
+            print(json.dumps(dict(element=name, slices=n, **errs)))
+        lines.append((name, rows))
+        lat.close()
+    if args.out:
+        with open(args.out, "w") as f:
+            f.write("# Single-element spin errors against the number of slices (the paper's Fig. 7, P:648-660), computed on the GPU\n\n")
+            f.write("Command: `python -m paper_1501_03450_b200.studies fig7`\n\n")
+            f.write("|S - S_ref| for the test particle of footnote 5; S_ref = 256 slices, three Romberg iterations (P:652).  PWC = mid-slice\n"
+                    "piece-wise constant (37); k = Romberg iterations on the slice-edge products (38)(39), k = 0 is the trapezoid product.\n\n")
+            for name, rows in lines:
+                f.write("## %s\n\n| slices | PWC | k = 0 | k = 1 | k = 2 | k = 3 |\n|---|---|---|---|---|---|\n" % name)
+                for n, e in rows:
+                    f.write("| %d | %s |\n" % (n, " | ".join("%.2e" % e[k] if e[k] is not None else "" for k in ("pwc", "k0", "k1", "k2", "k3"))))
+                f.write("\n")
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     sub = ap.add_subparsers(dest="study", required=True)
@@ -157,9 +223,11 @@ def main(argv=None):
     s.add_argument("--order4", action="store_true",
                    help="add the fourth-order compositions (SURVEY 8(f) f1); the reference becomes matrix_kick_4")
     s.add_argument("--out", default=None)
+    g = sub.add_parser("fig7")
+    g.add_argument("--out", default=None)
     args = ap.parse_args(argv)
     t0 = time.time()
-    (ramp if args.study == "ramp" else sweep)(args)
+    {"ramp": ramp, "sweep": sweep, "fig7": fig7}[args.study](args)
     print(json.dumps(dict(wall_s=time.time() - t0)))
 
 

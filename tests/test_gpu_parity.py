@@ -371,6 +371,27 @@ def test_chain_rotation_edge_sizes(gst, n, turns):
     assert np.array_equal(rot[0], sta[0]) and rot[4] == sta[4]
 
 
+def test_fig7_claims_through_the_c_abi(gst, capsys):
+    """The paper's single-element study run on the GPU (studies.fig7): slope -2 without Romberg, slope -4
+    with one iteration, and for the IR quadrupole "four slices plus two Romberg iterations yield a
+    four-decade reduction"."""
+    import argparse
+    import json
+    from paper_1501_03450_b200 import studies
+    studies.fig7(argparse.Namespace(out=None))
+    rows = [json.loads(l) for l in capsys.readouterr().out.splitlines() if l.startswith("{")]
+    quad = {r["slices"]: r for r in rows if r["element"].startswith("IR quadrupole")}
+    dip = {r["slices"]: r for r in rows if r["element"].startswith("arc dipole")}
+    for tab in (quad, dip):
+        for n in (4, 8, 16):
+            assert 3.5 < tab[n]["pwc"] / tab[2 * n]["pwc"] < 4.5 and 3.5 < tab[n]["k0"] / tab[2 * n]["k0"] < 4.5
+    for n in (8, 16, 32):
+        assert 13 < quad[n]["k1"] / quad[2 * n]["k1"] < 19
+    assert 14 < dip[16]["k1"] / dip[32]["k1"] < 19 and 14 < dip[32]["k1"] / dip[64]["k1"] < 19
+    assert quad[4]["k2"] < 2e-4 * quad[4]["k0"]                     # four decades
+    assert min(quad[128]["k3"], dip[128]["k3"]) < 1e-14            # round-off floor ~1e-15
+
+
 def test_chunked_tracking_is_bit_identical_to_one_call(gst):
     lat = mixed_lattice(ramp=True)
     bm = W.beam(12.0)
