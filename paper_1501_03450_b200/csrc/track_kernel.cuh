@@ -167,7 +167,7 @@ __device__ __forceinline__ void pcon_set(PCon& c, double Pt, const Ref& r, doubl
 // operand (a double literal would cost two extra UMOV/MOV instructions per use on sm_100).
 //   QPOLY[2k]   = (-1/4)^k/(2k)!        (cos x,        x^2 = v/4)
 //   QPOLY[2k+1] = (1/2)(-1/4)^k/(2k+1)!  (sin(x)/th)
-__constant__ double QPOLY[14] = {
+static __constant__ double QPOLY[14] = {
     1.0, 0.5,
     -1.0 / 8.0, -0.5 / 24.0,
     1.0 / (16.0 * 24.0), 0.5 / (16.0 * 120.0),
@@ -178,7 +178,7 @@ __constant__ double QPOLY[14] = {
 
 // tiers 2 and 3 (large angle per edge), kept out of line: they are rare and would otherwise be
 // replicated at every call site (instruction-cache footprint)
-__device__ __noinline__ double2 quat_cs_slow(double v) {
+static __device__ __noinline__ double2 quat_cs_slow(double v) {
   double c, s;
   if (v <= 2.0) {
     // tier 2: u = v/4 <= 0.5, k = 0..9, remainder < 4e-20
@@ -248,7 +248,7 @@ __device__ __forceinline__ void quat_rotate(const Quat& q, double& Sx, double& S
 // The Romberg table (39b) is linear in its first column, so its bottom-right entry is a fixed linear
 // combination of the DEPTH level products: row d-1 holds the weights of Q[0] (finest) .. Q[d-1] (coarsest),
 // obtained by running (39b) on unit vectors (exact integers over a common denominator).
-__constant__ double ROMBERG_W[6][6] = {
+static __constant__ double ROMBERG_W[6][6] = {
     {1.0, 0.0, 0.0, 0.0, 0.0, 0.0},
     {4.0 / 3.0, -1.0 / 3.0, 0.0, 0.0, 0.0, 0.0},
     {64.0 / 45.0, -20.0 / 45.0, 1.0 / 45.0, 0.0, 0.0, 0.0},
@@ -480,7 +480,7 @@ struct BendExact {
   }
 };
 
-__constant__ double APOLY[6] = {1.0 / 6.0, 3.0 / 40.0, 15.0 / 336.0, 105.0 / 3456.0, 945.0 / 42240.0, 10395.0 / 599040.0};
+static __constant__ double APOLY[6] = {1.0 / 6.0, 3.0 / 40.0, 15.0 / 336.0, 105.0 / 3456.0, 945.0 / 42240.0, 10395.0 / 599040.0};
 
 // asin(x): polynomial for the small arguments of differences of nearby angles, the library routine otherwise
 __device__ __forceinline__ double asin_small(double x) {
@@ -1015,7 +1015,7 @@ __device__ __forceinline__ bool solenoid(State& z, const DevElem& e, const PCon&
   return !s.bad;
 }
 
-__constant__ double FRINGE_INV_M[4] = {1.0 / 2.0, 1.0 / 3.0, 1.0 / 4.0, 1.0 / 5.0};
+static __constant__ double FRINGE_INV_M[4] = {1.0 / 2.0, 1.0 / 3.0, 1.0 / 4.0, 1.0 / 5.0};
 
 // The tests are ordered by how often each type occurs in a ring (drifts, quadrupoles, bends, thin lenses).
 template <int SPLIT, int ORDER, class Spin>
