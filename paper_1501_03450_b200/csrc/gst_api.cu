@@ -386,7 +386,6 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   a.G = lat->beam.G;
   size_t tab_bytes = lat->uniq.size() * sizeof(gst::DevElem);
   size_t seq_bytes = (lat->seq.size() * sizeof(uint32_t) + 15) & ~size_t(15);
-  if (tab_bytes > 24 * 1024) return fail(GST_EINVAL, "too many unique elements for the shared-memory table (%zu)", lat->uniq.size());
   const bool pair = g_variant.load() == GST_KERNEL_PAIR;
   gst::ChainLaunch chain_req;
   chain_req.args.sm_scratch = b->d_chain_flag;
@@ -396,6 +395,7 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   chain_req.steps_per_turn = gst_lattice_steps_per_turn(lat, table_slices);
   gst::ChainLaunch* chain = g_variant.load() == GST_KERNEL_FUSED ? &chain_req : nullptr;
   a.use_smem_seq = 0;
+  a.use_smem_tab = 0;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   cudaError_t ce;
   const int order = (int)split >= 3 ? 4 : 2;

@@ -53,15 +53,21 @@ __device__ __forceinline__ void st_release(int* p, int v) {
 template <int SPLIT, int DEPTH, int ORDER>
 __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_chain_kernel(const TrackArgs a, const ChainArgs ch) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  DevElem* tab = reinterpret_cast<DevElem*>(smem_raw);
+  // a0: stage the unique-element table and the sequence into shared memory, each when it fits
+  const DevElem* tab = a.tab;
   const uint32_t* seq = a.seq;
   {
-    const int nw = a.n_unique * (int)(sizeof(DevElem) / sizeof(double));
-    const double* src = reinterpret_cast<const double*>(a.tab);
-    double* dst = reinterpret_cast<double*>(smem_raw);
-    for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
+    size_t off = 0;
+    if (a.use_smem_tab) {
+      const int nw = a.n_unique * (int)(sizeof(DevElem) / sizeof(double));
+      const double* src = reinterpret_cast<const double*>(a.tab);
+      double* dst = reinterpret_cast<double*>(smem_raw);
+      for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
+      tab = reinterpret_cast<const DevElem*>(smem_raw);
+      off = (size_t)a.n_unique * sizeof(DevElem);
+    }
     if (a.use_smem_seq) {
-      uint32_t* sseq = reinterpret_cast<uint32_t*>(smem_raw + (size_t)a.n_unique * sizeof(DevElem));
+      uint32_t* sseq = reinterpret_cast<uint32_t*>(smem_raw + off);
       for (int i = threadIdx.x; i < a.n_seq; i += blockDim.x) sseq[i] = a.seq[i];
       seq = sseq;
     }

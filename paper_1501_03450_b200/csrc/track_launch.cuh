@@ -31,11 +31,14 @@ cudaError_t launch_split_mk(int order, int depth, const TrackArgs& a, size_t tab
 namespace {
 
 // shared memory of one block: [ring + lost flags (pair kernel only)] table [sequence when it fits]
-struct SmemPlan { size_t bytes; int use_smem_seq; };
+struct SmemPlan { size_t bytes; int use_smem_tab, use_smem_seq; };
 SmemPlan plan_smem(size_t tab_bytes, size_t seq_bytes, size_t fixed, size_t budget) {
   SmemPlan p;
-  p.use_smem_seq = (fixed + tab_bytes + seq_bytes <= budget) ? 1 : 0;
-  p.bytes = fixed + tab_bytes + (p.use_smem_seq ? seq_bytes : 0);
+  // the table first (read at every element), then the sequence; what does not fit stays in global memory
+  p.use_smem_tab = (fixed + tab_bytes <= budget) ? 1 : 0;
+  const size_t with_tab = fixed + (p.use_smem_tab ? tab_bytes : 0);
+  p.use_smem_seq = (with_tab + seq_bytes <= budget) ? 1 : 0;
+  p.bytes = with_tab + (p.use_smem_seq ? seq_bytes : 0);
   return p;
 }
 
@@ -79,6 +82,8 @@ cudaError_t launch_track(TrackArgs a, size_t tab_bytes, size_t seq_bytes, bool p
     SmemPlan p = plan_smem(tab_bytes, seq_bytes, fixed, budget);
 
     a.use_smem_seq = p.use_smem_seq;
+  a.use_smem_tab = p.use_smem_tab;
+    a.use_smem_tab = p.use_smem_tab;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
     if (e != cudaSuccess) return e;
     // ask for just enough shared memory for MIN_BLOCKS blocks; the rest of the 228 kB stays L1
@@ -94,6 +99,7 @@ cudaError_t launch_track(TrackArgs a, size_t tab_bytes, size_t seq_bytes, bool p
   }
   SmemPlan p = plan_smem(tab_bytes, seq_bytes, 0, 24 * 1024);
   a.use_smem_seq = p.use_smem_seq;
+  a.use_smem_tab = p.use_smem_tab;
   if constexpr (ORDER == 2 && DEPTH >= 1) {
     if (chain) {   // T1c: the same kernel with the chains rotating over all resident warp slots
       auto ck = track_chain_kernel<SPLIT, DEPTH, ORDER>;

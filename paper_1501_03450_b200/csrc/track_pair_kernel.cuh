@@ -229,15 +229,20 @@ __global__ void __launch_bounds__(PairCfg<DEPTH>::THREADS, PairCfg<DEPTH>::MIN_B
   double* ring = reinterpret_cast<double*>(smem_raw);
   uint8_t* flag = smem_raw + PAIRS * PAIR_RING_BYTES;
   unsigned char* tab_raw = flag + PAIRS * 32;
-  DevElem* tab = reinterpret_cast<DevElem*>(tab_raw);
+  const DevElem* tab = a.tab;
   const uint32_t* seq = a.seq;
   {
-    const int nw = a.n_unique * (int)(sizeof(DevElem) / sizeof(double));
-    const double* src = reinterpret_cast<const double*>(a.tab);
-    double* dst = reinterpret_cast<double*>(tab_raw);
-    for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
+    size_t off = 0;
+    if (a.use_smem_tab) {
+      const int nw = a.n_unique * (int)(sizeof(DevElem) / sizeof(double));
+      const double* src = reinterpret_cast<const double*>(a.tab);
+      double* dst = reinterpret_cast<double*>(tab_raw);
+      for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
+      tab = reinterpret_cast<const DevElem*>(tab_raw);
+      off = (size_t)a.n_unique * sizeof(DevElem);
+    }
     if (a.use_smem_seq) {
-      uint32_t* sseq = reinterpret_cast<uint32_t*>(tab_raw + (size_t)a.n_unique * sizeof(DevElem));
+      uint32_t* sseq = reinterpret_cast<uint32_t*>(tab_raw + off);
       for (int i = threadIdx.x; i < a.n_seq; i += blockDim.x) sseq[i] = a.seq[i];
       seq = sseq;
     }

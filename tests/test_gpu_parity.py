@@ -392,6 +392,69 @@ def test_fig7_claims_through_the_c_abi(gst, capsys):
     assert min(quad[128]["k3"], dip[128]["k3"]) < 1e-14            # round-off floor ~1e-15
 
 
+@pytest.mark.parametrize("seed", range(8))
+def test_random_lattices_of_every_element_type(gst, O, seed):
+    """Seeded random lattices (every element type, random strengths, slice multipliers and order), a random split,
+    slicing and spin scheme each: the CUDA path against the oracle."""
+    rng = np.random.default_rng(1000 + seed)
+    u = lambda a, b: float(rng.uniform(a, b))
+    makers = [
+        lambda: W.drift(u(0.1, 2.0)),
+        lambda: W.quad(u(0.2, 0.8), u(0.03, 0.15) * rng.choice([-1, 1]), slice_mult=int(rng.integers(1, 3))),
+        lambda: W.sbend(u(0.5, 3.0), u(0.01, 0.05) * rng.choice([-1, 1]), eta=u(0.998, 1.002)),
+        lambda: W.rbend(u(0.5, 3.0), u(0.01, 0.05) * rng.choice([-1, 1])),
+        lambda: W.multipole(u(0.1, 0.5), kn=(u(-0.05, 0.05), u(-2, 2), u(-30, 30), u(-300, 300)),
+                            ks=(u(-0.05, 0.05), u(-2, 2), u(-30, 30), u(-300, 300))),
+        lambda: W.thin_multipole((u(-0.01, 0.01), u(-1, 1), u(-10, 10), u(-100, 100)), (u(-0.01, 0.01), u(-1, 1), u(-10, 10), u(-100, 100))),
+        lambda: W.solenoid(u(0.3, 1.5), u(0.05, 0.2) * rng.choice([-1, 1])),
+        lambda: W.fringe(float(rng.choice([-1, 1])), u(-0.05, 0.05), (u(-0.5, 0.5), u(-5, 5), 0.0, 0.0), (u(-0.5, 0.5), 0.0, 0.0, 0.0)),
+        lambda: W.snake(u(0.5, 3.1), u(-1.5, 1.5)),
+        lambda: W.cavity(u(1e4, 2e5), float(rng.integers(1, 20)), u(-0.3, 0.3), float(rng.choice([-1, 1]))),
+        lambda: W.marker(),
+    ]
+    els = [makers[int(rng.integers(len(makers)))]() for _ in range(44)]     # 44 unique records: over the shared-memory table
+    lat = W.lattice(els)
+    gam = u(3.0, 30.0)
+    bm = W.beam(gam)
+    st = W.gaussian_bunch(2000 + seed, 150, gam, 1e-3, 1e-4, 1e-3, 1e-4, 5e-4, 0.05, "sphere")
+    split = int(rng.integers(0, 6))
+    depth = int(rng.choice([-1, 0, 1, 2, 3, 4])) if split < 3 else int(rng.integers(1, 5))
+    n_slices = (1 << max(depth - 1, 0)) * int(rng.integers(1, 4))
+    ref, rlost, g_ref = O.track(lat, bm, st, 2, split, n_slices, depth)
+    got, lost, pol, emit, g_gpu = gpu_track(gst, lat, bm, st, 2, split, n_slices, depth)
+    assert np.array_equal(lost.astype(bool), rlost.astype(bool))
+    keep = ~rlost.astype(bool)
+    assert keep.sum() >= 140
+    # a random lattice is not a stable ring: two turns amplify rounding differences more than the FODO-like lattices do
+    assert orbit_err(got[:, keep], ref[:, keep]) < 2e-11, (split, depth, n_slices, orbit_err(got[:, keep], ref[:, keep]))
+    assert spin_err(got[:, keep], ref[:, keep]) < 2e-11, (split, depth, n_slices, spin_err(got[:, keep], ref[:, keep]))
+    assert abs(g_gpu - g_ref) < 1e-12 * g_ref
+
+
+def test_lattice_with_hundreds_of_unique_elements(gst, O):
+    """A ring whose magnets all differ slightly (as a real machine's do): 448 unique records = 287 kB of element
+    table, read from global memory instead of shared memory; the sequence alone still fits."""
+    rng = np.random.default_rng(77)
+    els = []
+    for e in W.fodo_ring(64):
+        e = e.copy()
+        if int(e["type"]) == W.QUAD:
+            e["kn"][0] *= 1.0 + 1e-3 * rng.standard_normal()
+        elif int(e["type"]) == W.SBEND:
+            e["k0"] *= 1.0 + 1e-4 * rng.standard_normal()
+        else:
+            e["L"] *= 1.0 + 1e-3 * rng.standard_normal()
+        els.append(e)
+    lat = W.lattice(els)
+    assert len(np.unique(lat)) > 400
+    bm = W.beam(25.0)
+    st = W.gaussian_bunch(41, 96, 25.0, 1e-3, 1e-4, 1e-3, 1e-4, 3e-4, 0.05, "sphere")
+    ref, rlost, _ = O.track(lat, bm, st, 3, W.SPLIT_MATRIX_KICK, 4, 3)
+    got, lost, pol, emit, _ = gpu_track(gst, lat, bm, st, 3, W.SPLIT_MATRIX_KICK, 4, 3)
+    assert not rlost.any() and not lost.any()
+    assert orbit_err(got, ref) < 5e-12 and spin_err(got, ref) < 5e-12, (orbit_err(got, ref), spin_err(got, ref))
+
+
 def test_chunked_tracking_is_bit_identical_to_one_call(gst):
     lat = mixed_lattice(ramp=True)
     bm = W.beam(12.0)
