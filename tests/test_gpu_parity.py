@@ -455,6 +455,23 @@ def test_lattice_with_hundreds_of_unique_elements(gst, O):
     assert orbit_err(got, ref) < 5e-12 and spin_err(got, ref) < 5e-12, (orbit_err(got, ref), spin_err(got, ref))
 
 
+def test_long_lattice_whose_sequence_does_not_fit_shared_memory(gst, O):
+    """10 500 elements: the 42 kB sequence stays in global memory (prefetched one element ahead), the table is staged."""
+    lat = W.fodo_ring(1500)
+    assert len(lat) > 10000
+    bm = W.beam(25.0)
+    st = W.gaussian_bunch(43, 70, 25.0, 1e-3, 1e-4, 1e-3, 1e-4, 3e-4, 0.05, "sphere")
+    for variant in (gst.KERNEL_FUSED, gst.KERNEL_PAIR):
+        ref, rlost, _ = O.track(lat, bm, st, 1, W.SPLIT_BEND_KICK, 2, 2)
+        try:
+            gst.set_kernel_variant(variant)
+            got, lost, pol, emit, _ = gpu_track(gst, lat, bm, st, 1, W.SPLIT_BEND_KICK, 2, 2)
+        finally:
+            gst.set_kernel_variant(gst.KERNEL_FUSED)
+        assert not rlost.any() and not lost.any()
+        assert orbit_err(got, ref) < 2e-11 and spin_err(got, ref) < 2e-11, (orbit_err(got, ref), spin_err(got, ref))
+
+
 def test_chunked_tracking_is_bit_identical_to_one_call(gst):
     lat = mixed_lattice(ramp=True)
     bm = W.beam(12.0)
