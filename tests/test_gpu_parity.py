@@ -472,6 +472,28 @@ def test_long_lattice_whose_sequence_does_not_fit_shared_memory(gst, O):
         assert orbit_err(got, ref) < 2e-11 and spin_err(got, ref) < 2e-11, (orbit_err(got, ref), spin_err(got, ref))
 
 
+def test_two_bunches_on_two_streams(gst):
+    """Two gst_track calls in flight on different streams (both take the cooperative sequence launch, which needs
+    the whole chip): they serialise instead of dead-locking, and give the single-stream results."""
+    lat = mixed_lattice(ramp=True)
+    bm = W.beam(12.0)
+    sts = [W.gaussian_bunch(50 + k, 65536, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere") for k in range(2)]
+    want = [gpu_track(gst, lat, bm, st, 32, W.SPLIT_BEND_KICK, 4, 3)[0] for st in sts]
+    L = gst.Lattice(lat, bm)
+    devs = [torch.tensor(st, dtype=torch.float64, device="cuda").contiguous() for st in sts]
+    bunches = [gst.Bunch(d) for d in devs]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    for b, s in zip(bunches, streams):
+        b.track(L, 32, W.SPLIT_BEND_KICK, 4, 3, stream=s)
+    torch.cuda.synchronize()
+    for b, d, w in zip(bunches, devs, want):
+        assert b.last_kernel() == "track_chain_kernel"
+        assert np.array_equal(d.cpu().numpy(), w)
+        b.close()
+    L.close()
+
+
 def test_chunked_tracking_is_bit_identical_to_one_call(gst):
     lat = mixed_lattice(ramp=True)
     bm = W.beam(12.0)
