@@ -72,11 +72,13 @@ typedef enum {
 typedef struct {
   int32_t type;       /* gst_elem_type                                                            */
   int32_t slice_mult; /* thick magnets: slices = n_slices * slice_mult ("4 n_b"); >= 1      */
-  double L;           /* length [m]; > 0 for DRIFT/SBEND/QUAD/MULTIPOLE, ignored otherwise        */
+  double L;           /* length [m]; > 0 for DRIFT/SBEND/QUAD/MULTIPOLE/SOLENOID/RBEND, ignored otherwise */
   double h;           /* SBEND: curvature of the local frame 1/rho_c = angle/L [1/m]; != 0 */
-  double k0;          /* SBEND: b1/(B rho)_o = eta*h [1/m] (9); eta != 1 is a mis-powered magnet  */
+  double k0;          /* SBEND: b1/(B rho)_o = eta*h [1/m] (9); eta != 1 is a mis-powered magnet;
+                         RBEND: 1/rho_b; SOLENOID: b_0/(B rho)_o; FRINGE: the magnet's dipole strength   */
   double kn[4];       /* normal  b_m/(B rho)_o, m = 2..5 -> kn[m-2], convention of (28): no 1/(m-1)!;
-                         QUAD uses kn[0] only (!= 0); THINMULT: integrated (times L)             */
+                         QUAD uses kn[0] only (!= 0); THINMULT: integrated (times L);
+                         RBEND: kn[0] = phi_entr, kn[1] = phi_exit [rad]                          */
   double ks[4];       /* skew    a_m/(B rho)_o, same layout; must be 0 for QUAD                   */
   double volt_eV;     /* RFCAV: q*V peak energy gain [eV]                                         */
   double harmonic;    /* RFCAV: harmonic number; k_rf = 2 pi harmonic beta_o / C, C = sum of L    */
@@ -99,7 +101,8 @@ typedef struct gst_bunch gst_bunch;
 /* Stage an element table (a0).  `elems` and `beam` are HOST pointers, copied.  The table is
  * de-duplicated to unique elements + a uint16 sequence and uploaded to the current CUDA device.
  * GST_EINVAL: n == 0, unknown type, L <= 0 for a thick element, SBEND with h == 0 or k0 == 0, QUAD
- * with kn[0] == 0 or any skew/higher term, slice_mult < 1, more than 65535 unique elements.      */
+ * with kn[0] == 0 or any skew/higher term, SOLENOID or RBEND with k0 == 0, RBEND whose angles do not
+ * match L*k0, slice_mult < 1, more than 65535 unique elements.                                    */
 gst_status gst_lattice_create(const gst_element* elems, size_t n, const gst_beam* beam, gst_lattice** out);
 void gst_lattice_destroy(gst_lattice* lat);
 
