@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_chain_ker
     PCon pc;
     pcon_set(pc, z.Pt, ref, a.G);
     bool lost = false;
-    typename SpinPolicy<DEPTH>::type spin(z);
+    typename SpinPolicy<DEPTH, SPLIT>::type spin(z);
     const long long t0 = k * ch.chunk_turns;
     const long long t1 = t0 + ch.chunk_turns < a.n_turns ? t0 + ch.chunk_turns : a.n_turns;
     uint32_t nxt = seq[0];
