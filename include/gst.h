@@ -170,7 +170,9 @@ gst_status gst_bunch_set_reference(gst_bunch* b, const gst_beam* beam, int64_t t
 
 /* End-to-end convenience with HOST buffers: allocates device arrays, copies the nine host arrays
  * (n doubles each, pinned or pageable) to the device, tracks, reduces, copies the state back into
- * the same host arrays and frees.  out_pol = {Px,Py,Ps,|P|}, out_lost may be NULL.  Synchronous.  */
+ * the same host arrays.  out_pol = {Px,Py,Ps,|P|}, out_lost may be NULL.  Synchronous.  The device
+ * workspace is kept in the lattice handle between calls of the same bunch size (freed by gst_lattice_destroy);
+ * concurrent calls on one lattice serialise.                                                          */
 gst_status gst_track_host(const gst_lattice* lat, double* const host_state[9], size_t n, int64_t n_turns,
                           gst_split split, int n_slices, int romberg_depth, double out_pol[4], int64_t* out_lost);
 

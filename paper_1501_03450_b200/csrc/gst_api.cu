@@ -57,6 +57,13 @@ struct gst_lattice {
   mutable std::map<int, DevTable> tables;   // derived unique-element tables, keyed by n_slices
   mutable std::mutex mu;
   std::vector<double> cav_dEs;      // per cavity in lattice order: volt*sin(phi_s)
+  // workspace of gst_track_host, kept between calls (device state, bunch handle, stream) so that the end-to-end
+  // call costs two copies and the kernels, not allocations; guarded by mu_host (calls on one lattice serialise)
+  mutable std::mutex mu_host;
+  mutable double* ws_state = nullptr;
+  mutable size_t ws_n = 0;
+  mutable gst_bunch* ws_bunch = nullptr;
+  mutable cudaStream_t ws_stream = nullptr;
 };
 
 struct gst_bunch {
@@ -281,6 +288,9 @@ gst_status gst_lattice_create(const gst_element* elems, size_t n, const gst_beam
 
 void gst_lattice_destroy(gst_lattice* lat) {
   if (!lat) return;
+  if (lat->ws_bunch) gst_bunch_destroy(lat->ws_bunch);
+  if (lat->ws_state) cudaFree(lat->ws_state);
+  if (lat->ws_stream) cudaStreamDestroy(lat->ws_stream);
   for (auto& kv : lat->tables) cudaFree(kv.second.d_tab);
   cudaFree(lat->d_seq);
   delete lat;
@@ -494,18 +504,30 @@ gst_status gst_track_host(const gst_lattice* lat, double* const host_state[9], s
   if (!lat || !host_state || !out_pol) return fail(GST_EINVAL, "null argument");
   gst_status vs = validate_track(lat, n_turns, (int)split, n_slices, romberg_depth);
   if (vs != GST_OK) return vs;
-  double* d = nullptr;
-  cudaStream_t st = nullptr;
-  CUDA_TRY(cudaMalloc(&d, sizeof(double) * 9 * (n ? n : 1)));
-  gst_bunch* b = nullptr;
+  std::lock_guard<std::mutex> lk(lat->mu_host);
+  if (!lat->ws_stream) CUDA_TRY(cudaStreamCreate(&lat->ws_stream));
+  if (!lat->ws_bunch || lat->ws_n != n) {          // (re)build the workspace for this bunch size
+    if (lat->ws_bunch) gst_bunch_destroy(lat->ws_bunch);
+    if (lat->ws_state) cudaFree(lat->ws_state);
+    lat->ws_bunch = nullptr;
+    lat->ws_state = nullptr;
+    CUDA_TRY(cudaMalloc(&lat->ws_state, sizeof(double) * 9 * (n ? n : 1)));
+    double* d0 = lat->ws_state;
+    gst_status bs = gst_bunch_init(d0, d0 + n, d0 + 2 * n, d0 + 3 * n, d0 + 4 * n, d0 + 5 * n, d0 + 6 * n, d0 + 7 * n,
+                                   d0 + 8 * n, n, &lat->ws_bunch);
+    if (bs != GST_OK) return bs;
+    lat->ws_n = n;
+  }
+  double* d = lat->ws_state;
+  cudaStream_t st = lat->ws_stream;
+  gst_bunch* b = lat->ws_bunch;
+  b->have_ref = false;                             // a fresh bunch every call: reference energy from the lattice, turn 0
+  b->turn = 0;
   gst_status s = GST_OK;
-  cudaError_t ce = cudaStreamCreate(&st);
-  if (ce != cudaSuccess) { cudaFree(d); return fail(GST_ECUDA, "cudaStreamCreate: %s", cudaGetErrorString(ce)); }
+  cudaError_t ce = cudaMemsetAsync(b->d_lost, 0, n > 0 ? n : 1, st);
   for (int i = 0; i < 9 && ce == cudaSuccess; ++i)
     ce = cudaMemcpyAsync(d + i * n, host_state[i], sizeof(double) * n, cudaMemcpyHostToDevice, st);
   if (ce != cudaSuccess) s = fail(GST_ECUDA, "H2D: %s", cudaGetErrorString(ce));
-  if (s == GST_OK)
-    s = gst_bunch_init(d, d + n, d + 2 * n, d + 3 * n, d + 4 * n, d + 5 * n, d + 6 * n, d + 7 * n, d + 8 * n, n, &b);
   if (s == GST_OK) s = gst_track(b, lat, n_turns, split, n_slices, romberg_depth, st);
   if (s == GST_OK) s = gst_polarization(b, st, out_pol, out_lost);
   if (s == GST_OK) {
@@ -514,9 +536,6 @@ gst_status gst_track_host(const gst_lattice* lat, double* const host_state[9], s
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
     if (ce != cudaSuccess) s = fail(GST_ECUDA, "D2H: %s", cudaGetErrorString(ce));
   }
-  if (b) gst_bunch_destroy(b);
-  cudaStreamDestroy(st);
-  cudaFree(d);
   return s;
 }
 
