@@ -27,6 +27,10 @@
 #pragma once
 #include "track_kernel.cuh"
 
+#ifndef GST_CHAIN_POLL_NS
+#define GST_CHAIN_POLL_NS 8192u
+#endif
+
 namespace gst {
 
 struct ChainArgs {
@@ -108,10 +112,15 @@ __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_chain_ker
   for (long long p = slot; p < total; p += slots) {
     const long long k = p / M, c = p - k * M;             // chunk k of chain c
     if (k > 0) {                                          // chunk k-1 of this chain is stored
+      // a chunk runs for milliseconds: poll with a back-off of up to GST_CHAIN_POLL_NS, so that the warps that wait
+      // (320 of the 2368 slots at any time for 65 536 particles) do not take issue slots from the ones that work
       int tries = 0;
+      unsigned ns = 256;
+#pragma unroll 1
       while (ld_acquire(ch.flag + c) < (int)k) {
-        __nanosleep(256);
-        if (++tries > (1 << 25)) { *ch.err = 1; return; }
+        __nanosleep(ns);
+        if (ns < GST_CHAIN_POLL_NS) ns *= 2;
+        if (++tries > (1 << 21)) { *ch.err = 1; return; }     // ~20 s: no chunk takes that long
       }
     }
     const long long j = c * 32 + lane;

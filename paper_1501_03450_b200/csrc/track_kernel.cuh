@@ -224,8 +224,8 @@ __device__ __forceinline__ Quat quat_mul(const Quat& a, const Quat& b) {
   Quat r;
   r.w = fma(a.w, b.w, -fma(a.x, b.x, fma(a.y, b.y, a.s * b.s)));
   r.x = fma(a.w, b.x, fma(a.x, b.w, fma(a.y, b.s, -a.s * b.y)));
-  r.y = fma(a.w, b.y, fma(a.y, b.w, fma(a.s, b.x, -a.x * b.s)));
-  r.s = fma(a.w, b.s, fma(a.s, b.w, fma(a.x, b.y, -a.y * b.x)));
+  r.y = fma(a.w, b.y, fma(-a.x, b.s, fma(a.y, b.w, a.s * b.x)));
+  r.s = fma(a.w, b.s, fma(a.x, b.y, fma(-a.y, b.x, a.s * b.w)));
   return r;
 }
 // same axis, twice the angle
