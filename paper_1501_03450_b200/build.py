@@ -12,7 +12,7 @@ OBJ = os.path.join(CSRC, "build")
 SRC = [os.path.join(CSRC, f) for f in ("gst_api.cu", "track_split_dk.cu", "track_split_bk.cu", "track_split_mk.cu")]
 DEPS = SRC + [os.path.join(CSRC, f) for f in ("track_kernel.cuh", "track_pair_kernel.cuh", "track_chain_kernel.cuh",
                                               "track_launch.cuh", "reduce_kernel.cuh")] + \
-    [os.path.join(os.path.dirname(HERE), "include", "gst.h")]
+    [os.path.join(os.path.dirname(HERE), "include", "gst.h"), os.path.abspath(__file__)]   # the flags live in this file
 OUT = os.path.join(HERE, "libgst.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
