@@ -412,6 +412,19 @@ def rhic_like_ring(gamma0, snakes=True, phi_s=0.0, chroma=(2.0, 2.0)):
     return lat, info
 
 
+def resonance_crossing_ring(dGg_per_turn, eps, k=45, phi=0.0):
+    """Isolated spin resonance with a known strength, crossed at a known rate (recipe for the
+    Froissart-Stora pin of the ramp): the 16-cell FODO ring, a cavity that adds
+    dGg_per_turn to G*gamma_o every turn (phi_s = asin(1/4), A13) and a thin partial snake of angle
+    mu = 2 pi eps about a horizontal axis (A14).  For the on-axis particle the one-turn spin map is
+    R_y(2 pi G gamma) R_n(mu), whose tune gap at integer G gamma is eps.  Starts at G gamma = k - 1/2;
+    returns (lattice, beam, turns to reach k + 1/2)."""
+    dE = dGg_per_turn * MASS_PROTON_EV / G_PROTON
+    els = list(fodo_ring(16, rf=cavity(4.0 * dE, 12.0, math.asin(0.25), +1.0)))
+    els.append(snake(2.0 * math.pi * eps, phi))
+    return lattice(els), beam((k - 0.5) / G_PROTON), int(round(1.0 / dGg_per_turn))
+
+
 # ------------------------------------------------------------------------------------------------
 # the five BASELINE.json configurations (1-based, as in SURVEY §8(d))
 # ------------------------------------------------------------------------------------------------

@@ -554,6 +554,26 @@ def test_config4_ramp_reduced(gst, O):
     assert np.max(np.abs(pol - rp)) < 1e-6
 
 
+def test_ramp_through_an_isolated_resonance(gst, O):
+    """Froissart-Stora crossing (tests/test_oracle_rf_reductions.py) on the CUDA path: particle 0 is on axis
+    and must land on the closed form; the rest of the bunch (betatron and momentum spread) must agree with the
+    oracle through the partial flip, bunch polarization within the north star's 1e-6 for ramp configs."""
+    dGg, eps = 2.5e-4, 4.2e-3
+    lat, bm, turns = W.resonance_crossing_ring(dGg, eps)
+    st = W.gaussian_bunch(21, 64, bm["gamma0"], 1e-3, 1e-4, 1e-3, 1e-4, 1e-4, 0.01)
+    st[:6, 0] = 0.0
+    ref, rlost, g_ref = O.track(lat, bm, st, turns, W.SPLIT_BEND_KICK, 4, 3)
+    got, lost, pol, emit, g_gpu = gpu_track(gst, lat, bm, st, turns, W.SPLIT_BEND_KICK, 4, 3)
+    assert not rlost.any() and not lost.any()
+    # gamma_o is summed turn by turn in fp64 (long double in the oracle): half an ulp per turn at worst
+    assert abs(g_gpu - g_ref) < turns * 1.2e-16 * g_ref and abs(W.G_PROTON * g_gpu - 45.5) < 1e-9
+    fs = 2 * math.exp(-math.pi ** 2 * eps ** 2 / dGg) - 1
+    assert abs(got[7, 0] - fs) < 0.02 and np.max(np.abs(got[:6, 0])) == 0.0, (got[7, 0], fs)
+    assert orbit_err(got, ref) < 1e-8 and spin_err(got, ref) < 1e-8, (orbit_err(got, ref), spin_err(got, ref))
+    rp, _ = O.polarization(ref)
+    assert np.max(np.abs(pol - rp)) < 1e-6
+
+
 @pytest.mark.parametrize("split", [W.SPLIT_DRIFT_KICK, W.SPLIT_BEND_KICK, W.SPLIT_MATRIX_KICK])
 def test_config5_sweep_points_reduced(gst, O, split):
     c = W.config(5, n_particles=128)

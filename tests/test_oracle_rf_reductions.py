@@ -3,6 +3,7 @@ the reductions (A18, A19) of the CPU oracle.  Beyond these pins the cavity is "p
 import math
 
 import numpy as np
+import pytest
 
 from oracle import oracle as O
 from paper_1501_03450_b200 import workloads as W
@@ -56,6 +57,47 @@ def test_ramp_reference_energy_and_adiabatic_damping():
     s0 = np.zeros((9, 1)); s0[7] = 1.0
     o2, _, _ = O.track(lat, bm, s0, 50, W.SPLIT_MATRIX_KICK, 2, 1, prec=O.PREC_QUAD)
     assert np.max(np.abs(o2[:6])) < 1e-25
+
+
+def test_ramp_longitudinal_area_scales_with_the_reference_momentum():
+    """A13 rescales Pt = (E - E0)/(p0 c) to the new p0 and leaves T alone: the (T, Pt) rms area of a short
+    bunch (linear motion about phi_s) shrinks as p0/p0' = (beta gamma)_0/(beta gamma)_1, i.e. the normalised
+    longitudinal emittance is the adiabatic invariant.  A missing or inverted Pt rescale leaves the ratio
+    at 1 or at (p0'/p0)."""
+    g0 = 25.0
+    bm = W.beam(g0)
+    volt, phi_s = 3e6, math.asin(0.25)
+    lat = W.fodo_ring(16, rf=W.cavity(volt, 12.0, phi_s, +1.0))
+    st = W.gaussian_bunch(12, 64, g0, 0.0, 0.0, 0.0, 0.0, 1e-4, 0.01)
+    out, lost, g1 = O.track(lat, bm, st, 1500, W.SPLIT_MATRIX_KICK, 2, 1, prec=O.PREC_DOUBLE)
+    assert not lost.any()
+
+    def area(s):
+        return math.sqrt(np.linalg.det(np.cov(s[4], s[5], bias=True)))
+
+    shrink = g0 * W.beta_of_gamma(g0) / (g1 * W.beta_of_gamma(g1))
+    assert shrink < 0.96
+    assert abs(area(out) / area(st) / shrink - 1) < 3e-3
+
+
+@pytest.mark.parametrize("dGg,eps", [(2.5e-4, 2e-3), (2.5e-4, 4.2e-3), (2.5e-4, 8e-3), (1e-3, 8.4e-3)])
+def test_ramp_through_an_isolated_resonance_follows_froissart_stora(dGg, eps):
+    """Polarization through the ramp (config 4's subject) against the textbook closed form: crossing an
+    isolated resonance of strength eps at the rate alpha = d(G gamma)/d(theta) leaves
+    Sy_f / Sy_i = 2 exp(-pi eps^2 / (2 alpha)) - 1 (Froissart and Stora, 1960).  The resonance is a thin
+    partial snake (tune gap eps at integer G gamma) in a planar ring, the particle is on axis, so the only
+    inputs are A13's gamma_o(n) in Omega (6b), the snake rotation (A14) and the bend precession.  The spin
+    still nutates by eps/(distance to the resonance) = 2 eps at the end of the run: tolerance 0.02."""
+    lat, bm, turns = W.resonance_crossing_ring(dGg, eps)
+    st = np.zeros((9, 1))
+    st[7] = 1.0
+    out, lost, g1 = O.track(lat, bm, st, turns, W.SPLIT_BEND_KICK, 4, 3, prec=O.PREC_DOUBLE)
+    assert not lost.any() and np.max(np.abs(out[:6])) == 0.0
+    assert abs(W.G_PROTON * g1 - 45.5) < 1e-9
+    alpha = dGg / (2 * math.pi)
+    fs = 2 * math.exp(-math.pi * eps ** 2 / (2 * alpha)) - 1
+    assert abs(out[7, 0] - fs) < 0.02, (out[7, 0], fs)
+    assert abs(np.linalg.norm(out[6:9, 0]) - 1) < 1e-10
 
 
 def test_polarization_and_emittance_against_numpy():
