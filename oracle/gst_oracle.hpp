@@ -20,8 +20,8 @@
 //
 // Parity status: every function here is pinned by tests/test_oracle_*.py EXCEPT the RF cavity
 // with ramp (rf_cavity, A12/A13) whose formulas are not in the paper: it is pinned only by the
-// small-amplitude synchrotron tune and the adiabatic-damping invariant; beyond that it is
-// "parity unpinned".
+// small-amplitude synchrotron tune, the adiabatic invariants (transverse and longitudinal) and the
+// Froissart-Stora crossing of a partial-snake resonance; beyond that it is "parity unpinned".
 #pragma once
 #include <cmath>
 #include <cstdint>

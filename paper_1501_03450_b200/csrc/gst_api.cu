@@ -74,7 +74,7 @@ struct gst_bunch {
   double* d_result = nullptr;     // [2*RED_WIDTH]
   double* h_result = nullptr;     // pinned
   bool have_ref = false;
-  double E0 = 0, mass = 0;
+  double E0 = 0, E0lo = 0, mass = 0;   // reference energy E0 + E0lo (gst::ref_energy_add)
   int64_t turn = 0;
   // chain rotation (track_chain_kernel.cuh): per-chain progress flags and reference energies, error word
   int* d_chain_flag = nullptr;
@@ -321,7 +321,7 @@ gst_status gst_bunch_init(double* x, double* px, double* y, double* py, double* 
   const size_t n_chains = (n + 31) / 32 + 1;
   // [sm scratch | chain flags], zeroed together before every rotating launch
   if (ce == cudaSuccess) ce = cudaMalloc(&b->d_chain_flag, sizeof(int) * (n_chains + 2 * gst::CHAIN_MAX_SMID + 1));
-  if (ce == cudaSuccess) ce = cudaMalloc(&b->d_chain_E0, sizeof(double) * n_chains);
+  if (ce == cudaSuccess) ce = cudaMalloc(&b->d_chain_E0, sizeof(double) * 2 * n_chains);
   if (ce == cudaSuccess) ce = cudaMalloc(&b->d_err, sizeof(int));
   if (ce == cudaSuccess) ce = cudaMemset(b->d_err, 0, sizeof(int));
   if (ce != cudaSuccess) {
@@ -357,6 +357,7 @@ const char* gst_bunch_last_kernel(const gst_bunch* b) { return b ? b->last_kerne
 gst_status gst_bunch_set_reference(gst_bunch* b, const gst_beam* beam, int64_t turn) {
   if (!b || !beam || !(beam->gamma0 > 1.0) || !(beam->mass_eV > 0.0)) return fail(GST_EINVAL, "bad reference");
   b->E0 = beam->gamma0 * beam->mass_eV;
+  b->E0lo = 0.0;
   b->mass = beam->mass_eV;
   b->turn = turn;
   b->have_ref = true;
@@ -375,6 +376,7 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   const int table_slices = depth_code >= 1 ? n_slices : 2 * n_slices;
   if (!b->have_ref) {
     b->E0 = lat->beam.gamma0 * lat->beam.mass_eV;
+    b->E0lo = 0.0;
     b->mass = lat->beam.mass_eV;
     b->have_ref = true;
   }
@@ -392,6 +394,7 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   a.n = (long long)b->n;
   a.n_turns = n_turns;
   a.E0 = b->E0;
+  a.E0lo = b->E0lo;
   a.mass = b->mass;
   a.G = lat->beam.G;
   size_t tab_bytes = lat->uniq.size() * sizeof(gst::DevElem);
@@ -417,10 +420,10 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   if (ce != cudaSuccess) return fail(GST_ECUDA, "track launch: %s", cudaGetErrorString(ce));
   b->last_kernel = pair && romberg_depth >= 1 && (int)split < 3 ? "track_pair_kernel"
                    : (chain_req.taken ? "track_chain_kernel" : "track_kernel");
-  // host-side bookkeeping of the reference energy: the same IEEE additions the kernel performs
+  // host-side bookkeeping of the reference energy: the same IEEE operations the kernel performs
   for (int64_t t = 0; t < n_turns; ++t)
     for (double dEs : lat->cav_dEs)
-      if (dEs != 0.0) b->E0 = b->E0 + dEs;
+      if (dEs != 0.0) gst::ref_energy_add(b->E0, b->E0lo, dEs);
   b->turn += n_turns;
   return GST_OK;
 }

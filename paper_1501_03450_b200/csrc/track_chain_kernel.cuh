@@ -39,7 +39,7 @@ struct ChainArgs {
   int n_sm;            // SMs in use = gridDim.x / blocks per SM
   int* sm_scratch;     // [2 * CHAIN_MAX_SMID + 1] blocks arrived per SM, rank + 1 per SM, SMs ranked; zeroed with flag[]
   int* flag;           // [n_chains] chunks completed, zeroed before the launch
-  double* E0;          // [n_chains] reference energy after the chain's last chunk
+  double* E0;          // [2 n_chains] reference energy after the chain's last chunk: E0 at [c], E0lo at [n_chains + c]
   int* err;            // set to 1 when a wait times out
 };
 
@@ -135,6 +135,7 @@ __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_chain_ker
     }
     Ref ref;
     ref_set(ref, k == 0 ? a.E0 : __ldcg(ch.E0 + c), a.mass);
+    ref.E0lo = k == 0 ? a.E0lo : __ldcg(ch.E0 + ch.n_chains + c);
     PCon pc;
     pcon_set(pc, z.Pt, ref, a.G);
     bool lost = false;
@@ -165,7 +166,10 @@ __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_chain_ker
         __stcg(a.p[6] + j, z.Sx); __stcg(a.p[7] + j, z.Sy); __stcg(a.p[8] + j, z.Ss);
       }
     }
-    if (lane == 0) __stcg(ch.E0 + c, ref.E0);
+    if (lane == 0) {
+      __stcg(ch.E0 + c, ref.E0);
+      __stcg(ch.E0 + ch.n_chains + c, ref.E0lo);
+    }
     __threadfence();
     __syncwarp();
     if (lane == 0) st_release(ch.flag + c, (int)k + 1);

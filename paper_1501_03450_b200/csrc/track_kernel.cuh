@@ -86,7 +86,7 @@ struct TrackArgs {
   int use_smem_tab;         // 0: the table is too big for shared memory and is read from global memory (L1-cached, uniform)
   long long n;
   long long n_turns;
-  double E0, mass, G;
+  double E0, E0lo, mass, G;   // reference energy = E0 + E0lo (compensated sum of the cavity gains)
 };
 
 // One sequence entry carries the element type next to the table index, so that the per-element dispatch
@@ -118,6 +118,7 @@ __device__ __forceinline__ double rsqrt_nr(double x) {
 // reference-particle and per-particle constants that change only when Pt or E0 changes
 struct Ref {
   double E0, mass, p0c, beta0, gamma0, ibeta0, ibg2;  // ibg2 = 1/(beta0 gamma0)^2 = 1/beta0^2 - 1
+  double E0lo;                                        // E0 + E0lo = exact sum of the gains so far (ref_energy_add)
 };
 struct PCon {
   double e0;    // P^2 - 1 = 2 Pt/beta0 + Pt^2                      (22)
@@ -134,6 +135,19 @@ struct PCon {
   bool d_valid;
 };
 
+// A13: E_o <- E_o + dE_s once per turn and cavity.  The spin phase of a turn is 2 pi G gamma_o, so rounding errors of
+// E_o that pile up over n turns grow as n^2 in the spin (7.6e-8 after 4000 turns against the long-double oracle,
+// tests/test_gpu_parity.py::test_ramp_through_an_isolated_resonance).  The sum is therefore carried as an unevaluated
+// pair (two-sum, renormalised): E0 is the correctly rounded exact sum at every turn, E0lo the remainder.
+__host__ __device__ __forceinline__ void ref_energy_add(double& E0, double& E0lo, double dEs) {
+  const double s = E0 + dEs;
+  const double bb = s - E0;
+  const double err = (E0 - (s - bb)) + (dEs - bb);   // s + err = E0 + dEs exactly
+  const double lo = E0lo + err;
+  const double hi = s + lo;
+  E0lo = lo - (hi - s);
+  E0 = hi;
+}
 __device__ __forceinline__ void ref_set(Ref& r, double E0, double mass) {
   r.E0 = E0; r.mass = mass;
   r.gamma0 = E0 / mass;
@@ -1066,7 +1080,9 @@ __device__ __forceinline__ bool element_step(int type, State& z, const DevElem& 
     double num = fma(ref.p0c, z.Pt, dE - e.dEs);
     if (e.dEs != 0.0) {
       double p0_old = ref.p0c;
-      ref_set(ref, ref.E0 + e.dEs, ref.mass);
+      double E0 = ref.E0;
+      ref_energy_add(E0, ref.E0lo, e.dEs);
+      ref_set(ref, E0, ref.mass);
       double sc = p0_old / ref.p0c;
       z.Px *= sc; z.Py *= sc;
     }
@@ -1137,6 +1153,7 @@ __global__ void __launch_bounds__(TRACK_BLOCK, track_min_blocks(SPLIT, ORDER)) t
   z.Sx = a.p[6][j]; z.Sy = a.p[7][j]; z.Ss = a.p[8][j];
   Ref ref;
   ref_set(ref, a.E0, a.mass);
+  ref.E0lo = a.E0lo;
   PCon pc;
   pcon_set(pc, z.Pt, ref, a.G);
   // The turn and element loops run to the end for every thread, so that their counters, the sequence

@@ -150,6 +150,7 @@ __device__ __forceinline__ void orbit_role(const TrackArgs& a, const DevElem* ta
   }
   Ref ref;
   ref_set(ref, a.E0, a.mass);
+  ref.E0lo = a.E0lo;
   PCon pc;
   pcon_set(pc, z.Pt, ref, a.G);
   bool lost = false;

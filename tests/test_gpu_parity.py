@@ -565,8 +565,9 @@ def test_ramp_through_an_isolated_resonance(gst, O):
     ref, rlost, g_ref = O.track(lat, bm, st, turns, W.SPLIT_BEND_KICK, 4, 3)
     got, lost, pol, emit, g_gpu = gpu_track(gst, lat, bm, st, turns, W.SPLIT_BEND_KICK, 4, 3)
     assert not rlost.any() and not lost.any()
-    # gamma_o is summed turn by turn in fp64 (long double in the oracle): half an ulp per turn at worst
-    assert abs(g_gpu - g_ref) < turns * 1.2e-16 * g_ref and abs(W.G_PROTON * g_gpu - 45.5) < 1e-9
+    # gamma_o(n): the CUDA path carries E_o as a compensated sum (ref_energy_add), so 4000 gains later it is still the
+    # correctly rounded value; a plain fp64 sum is 1.8e-13 off here and shifts the spin phases by 7.6e-8
+    assert abs(g_gpu - g_ref) < 4e-16 * g_ref and abs(W.G_PROTON * g_gpu - 45.5) < 1e-11
     fs = 2 * math.exp(-math.pi ** 2 * eps ** 2 / dGg) - 1
     assert abs(got[7, 0] - fs) < 0.02 and np.max(np.abs(got[:6, 0])) == 0.0, (got[7, 0], fs)
     assert orbit_err(got, ref) < 1e-8 and spin_err(got, ref) < 1e-8, (orbit_err(got, ref), spin_err(got, ref))
