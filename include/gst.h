@@ -164,7 +164,9 @@ const char* gst_bunch_last_kernel(const gst_bunch* b);
 /* Copy the lost flags (1 = lost) to HOST memory, n bytes; synchronises the stream.                */
 gst_status gst_bunch_lost(gst_bunch* b, void* cuda_stream, uint8_t* host_out);
 
-/* Reference Lorentz factor and turn counter the bunch carries (host-side bookkeeping of A13).    */
+/* Reference Lorentz factor and turn counter the bunch carries (host-side bookkeeping of A13).
+ * The reference energy is summed with a remainder term (two doubles), so gamma0 is the correctly
+ * rounded E_o(n)/m after any number of cavity passages; gst_bunch_set_reference clears the remainder. */
 gst_status gst_bunch_reference(const gst_bunch* b, double* gamma0, int64_t* turn);
 gst_status gst_bunch_set_reference(gst_bunch* b, const gst_beam* beam, int64_t turn);
 
