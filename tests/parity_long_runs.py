@@ -27,7 +27,7 @@ def main():
     from paper_1501_03450_b200 import gst
     from paper_1501_03450_b200 import workloads as W
     rows = []
-    for cfg_i, turns in ((2, 1000), (3, 1000), (4, 1000), (5, 100)):
+    for cfg_i, turns in ((2, 1000), (3, 1000), (4, 5000), (5, 100)):
         c = W.config(cfg_i, n_particles=args.particles)
         st = c["state"]
         t0 = time.time()
