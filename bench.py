@@ -176,6 +176,7 @@ def main():
     import torch.distributed as dist
     from paper_1501_03450_b200 import distributed as D
     from paper_1501_03450_b200 import gst
+    from paper_1501_03450_b200 import gst_diag
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -271,11 +272,11 @@ def main():
     fm = load_flop_model()
     key = "%s_%s_n%d_d%d" % (cfg["name"], W.SPLIT_NAMES[split], n_slices, depth)
     flop_pt = fm.get(key, {}).get("flop_per_particle_turn")
-    peak_meas, peak_ms = gst.fp64_peak()
-    peak_rrr, _ = gst.fp64_peak_rrr()
+    peak_meas, peak_ms = gst_diag.fp64_peak()
+    peak_rrr, _ = gst_diag.fp64_peak_rrr()
     k_ms = float(np.mean(track_ms))
     roof = {"bound": "alu", "unit": "TFLOP/s", "kernel": "gst::%s<%d,%d,2>" % (bunch.last_kernel(), split, depth),
-            "kernel_ms": k_ms, "peak": peak_meas, "peak_kind": "measured DFMA chains (gst_fp64_peak), this run",
+            "kernel_ms": k_ms, "peak": peak_meas, "peak_kind": "measured DFMA chains (gst_diag_fp64_peak), this run",
             "peak_nominal": NOMINAL_FP64_TFLOPS,
             "peak_three_register_dfma": peak_rrr,   # context: DFMA R,R,R takes 3 cycles on B200
             "traffic": fm.get(key, {}).get("dram_bytes_per_launch"),

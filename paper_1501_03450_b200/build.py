@@ -1,7 +1,7 @@
 """Compile the CUDA C-ABI library in-tree: paper_1501_03450_b200/libgst.so (sm_100a only).
 
 The kernel instantiations of each split live in their own translation unit (csrc/track_split_*.cu) so that the
-four nvcc runs go in parallel; objects are kept under csrc/build/ (git-ignored)."""
+nvcc runs go in parallel; objects are kept under csrc/build/ (git-ignored)."""
 import os
 import subprocess
 import sys
@@ -9,10 +9,11 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
-SRC = [os.path.join(CSRC, f) for f in ("gst_api.cu", "track_split_dk.cu", "track_split_bk.cu", "track_split_mk.cu")]
-DEPS = SRC + [os.path.join(CSRC, f) for f in ("track_kernel.cuh", "track_pair_kernel.cuh", "track_chain_kernel.cuh",
-                                              "track_launch.cuh", "reduce_kernel.cuh")] + \
-    [os.path.join(os.path.dirname(HERE), "include", "gst.h"), os.path.abspath(__file__)]   # the flags live in this file
+SRC = [os.path.join(CSRC, f) for f in ("gst_api.cu", "gst_diag.cu", "track_split_dk.cu", "track_split_bk.cu", "track_split_mk.cu")]
+DEPS = SRC + [os.path.join(CSRC, f) for f in ("track_kernel.cuh", "track_chain_kernel.cuh", "track_launch.cuh",
+                                              "reduce_kernel.cuh", "gst_internal.h")] + \
+    [os.path.join(os.path.dirname(HERE), "include", f) for f in ("gst.h", "gst_diag.h")] + \
+    [os.path.abspath(__file__)]   # the flags live in this file
 OUT = os.path.join(HERE, "libgst.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]

@@ -1,6 +1,7 @@
 // gst_api.cu -- C ABI (include/gst.h) over the CUDA kernels: lattice staging (a0), bunch handles,
-// the track launch (T1), reductions (T2) and the FP64-peak microbenchmark (T3).
+// the track launch (T1) and the reductions (T2).  The diagnostics of include/gst_diag.h are in gst_diag.cu.
 #include "../../include/gst.h"
+#include "../../include/gst_diag.h"
 
 #include <cuda_runtime.h>
 
@@ -9,6 +10,7 @@
 #include <atomic>
 #include <cstdarg>
 #include <cstdio>
+#include <climits>
 #include <cstring>
 #include <map>
 #include <mutex>
@@ -16,13 +18,12 @@
 #include <string>
 #include <vector>
 
+#include "gst_internal.h"
 #include "reduce_kernel.cuh"
 #include "track_launch.cuh"
 
-namespace {
-
+namespace gst {
 thread_local std::string g_err = "";
-std::atomic<int> g_variant{GST_KERNEL_FUSED};
 
 gst_status fail(gst_status s, const char* fmt, ...) {
   char buf[512];
@@ -33,16 +34,19 @@ gst_status fail(gst_status s, const char* fmt, ...) {
   g_err = buf;
   return s;
 }
-#define CUDA_TRY(expr)                                                                      \
-  do {                                                                                      \
-    cudaError_t e_ = (expr);                                                                \
-    if (e_ != cudaSuccess) return fail(GST_ECUDA, "%s: %s", #expr, cudaGetErrorString(e_)); \
-  } while (0)
+}  // namespace gst
+
+namespace {
+using gst::DeviceGuard;
+using gst::fail;
 
 bool is_thick(int t) { return t == GST_SBEND || t == GST_QUAD || t == GST_MULTIPOLE || t == GST_SOLENOID || t == GST_RBEND; }
 
+// one derived unique-element table (a value of n_slices): pinned host copy, device copy, upload event
 struct DevTable {
+  gst::DevElem* h_tab = nullptr;
   gst::DevElem* d_tab = nullptr;
+  cudaEvent_t ready = nullptr;
 };
 
 }  // namespace
@@ -52,6 +56,8 @@ struct gst_lattice {
   std::vector<gst_element> uniq;    // de-duplicated
   std::vector<uint32_t> seq;        // gst::seq_pack(index into uniq, type) per lattice position
   gst_beam beam;
+  int device = 0;                   // the CUDA device the tables live on
+  int sms = 0;                      // its SM count
   double C = 0;                     // circumference = sum of L
   uint32_t* d_seq = nullptr;
   mutable std::map<int, DevTable> tables;   // derived unique-element tables, keyed by n_slices
@@ -69,6 +75,9 @@ struct gst_lattice {
 struct gst_bunch {
   double* p[9];
   size_t n = 0;
+  int device = 0;                 // the CUDA device that owns the arrays
+  gst_launch_mode launch_mode = GST_LAUNCH_AUTO;
+  long long poll_limit_override = 0;   // gst_diag_chain_poll_limit
   uint8_t* d_lost = nullptr;
   double* d_partials = nullptr;   // [RED_MAX_BLOCKS][RED_WIDTH]
   double* d_result = nullptr;     // [2*RED_WIDTH]
@@ -76,10 +85,11 @@ struct gst_bunch {
   bool have_ref = false;
   double E0 = 0, E0lo = 0, mass = 0;   // reference energy E0 + E0lo (gst::ref_energy_add)
   int64_t turn = 0;
-  // chain rotation (track_chain_kernel.cuh): per-chain progress flags and reference energies, error word
-  int* d_chain_flag = nullptr;
+  // chain rotation (track_chain_kernel.cuh): [scratch | per-chain progress flags], per-chain reference energies
+  int* d_chain = nullptr;
   double* d_chain_E0 = nullptr;
-  int* d_err = nullptr;
+  int* d_err = nullptr;           // error word: set by a kernel that gave up, cleared when the host has reported it
+  int* h_err = nullptr;           // pinned landing place of its copies
   const char* last_kernel = "";
 };
 
@@ -177,47 +187,62 @@ gst::DevElem derive(const gst_element& e, int n_slices, double C) {
   return d;
 }
 
-gst_status get_table(const gst_lattice* lat, int n_slices, const gst::DevElem** out) {
+// The derived table of one slicing: made on first use, uploaded on the caller's stream from a pinned copy that the
+// lattice keeps alive; `ready` orders every other stream behind that upload.
+gst_status get_table(const gst_lattice* lat, int n_slices, cudaStream_t st, const gst::DevElem** out) {
   std::lock_guard<std::mutex> lk(lat->mu);
   auto it = lat->tables.find(n_slices);
   if (it == lat->tables.end()) {
-    std::vector<gst::DevElem> host(lat->uniq.size());
-    for (size_t i = 0; i < lat->uniq.size(); ++i) host[i] = derive(lat->uniq[i], n_slices, lat->C);
+    const size_t bytes = lat->uniq.size() * sizeof(gst::DevElem);
     DevTable t;
-    CUDA_TRY(cudaMalloc(&t.d_tab, host.size() * sizeof(gst::DevElem)));
-    CUDA_TRY(cudaMemcpy(t.d_tab, host.data(), host.size() * sizeof(gst::DevElem), cudaMemcpyHostToDevice));
+    cudaError_t ce = cudaMallocHost(&t.h_tab, bytes);
+    if (ce == cudaSuccess) {
+      for (size_t i = 0; i < lat->uniq.size(); ++i) t.h_tab[i] = derive(lat->uniq[i], n_slices, lat->C);
+      ce = cudaMalloc(&t.d_tab, bytes);
+    }
+    if (ce == cudaSuccess) ce = cudaEventCreateWithFlags(&t.ready, cudaEventDisableTiming);
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(t.d_tab, t.h_tab, bytes, cudaMemcpyHostToDevice, st);
+    if (ce == cudaSuccess) ce = cudaEventRecord(t.ready, st);
+    if (ce != cudaSuccess) {
+      if (t.ready) cudaEventDestroy(t.ready);
+      if (t.d_tab) cudaFree(t.d_tab);
+      if (t.h_tab) cudaFreeHost(t.h_tab);
+      return fail(ce == cudaErrorMemoryAllocation ? GST_ENOMEM : GST_ECUDA, "staging the element table: %s", cudaGetErrorString(ce));
+    }
     it = lat->tables.emplace(n_slices, t).first;
+  } else {
+    CUDA_TRY(cudaStreamWaitEvent(st, it->second.ready, 0));
   }
   *out = it->second.d_tab;
   return GST_OK;
 }
 
-// max relative error (in units of 2^-53) of the branch-free reciprocal / reciprocal square root
-__global__ void math_selftest_kernel(unsigned long long* out, int n) {
-  double worst_rcp = 0.0, worst_rsq = 0.0;
-  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-    double x = exp2(-2.0 + 4.0 * ((double)i + 0.37) / (double)n);     // [0.25, 4)
-    double r = gst::rcp_nr(x), q = gst::rsqrt_nr(x);
-    double er = fabs(fma(r, x, -1.0));                                 // |r x - 1|, exact residual
-    double eq = fabs(fma(q * q, x, -1.0)) * 0.5;                       // ~ |q sqrt(x) - 1|
-    worst_rcp = fmax(worst_rcp, er);
-    worst_rsq = fmax(worst_rsq, eq);
-  }
-  atomicMax(out, (unsigned long long)__double_as_longlong(worst_rcp));
-  atomicMax(out + 1, (unsigned long long)__double_as_longlong(worst_rsq));
-}
-
 gst_status validate_track(const gst_lattice* lat, int64_t n_turns, int split, int n_slices, int depth) {
   if (n_turns < 0) return fail(GST_EINVAL, "n_turns < 0");
   if (split < 0 || split > 5) return fail(GST_EINVAL, "unknown split %d", split);
-  if (n_slices < 1 || n_slices > (1 << 20)) return fail(GST_EINVAL, "n_slices must be >= 1");
+  if (n_slices < 1 || n_slices > (1 << 20)) return fail(GST_EINVAL, "n_slices must be in 1..2^20");
   if (depth < 1 || depth > 6) return fail(GST_EINVAL, "romberg_depth must be in 1..6");
   for (const gst_element& e : lat->uniq)
     if (is_thick(e.type)) {
-      long N = (long)n_slices * e.slice_mult;
-      if (N % (1L << (depth - 1)) != 0)
-        return fail(GST_EINVAL, "2^(depth-1) = %ld does not divide the %ld slices of a thick element", 1L << (depth - 1), N);
+      const int64_t N = (int64_t)n_slices * e.slice_mult;          // 2 N must fit an int (half slices of gst_track_pwc)
+      if (N > (int64_t)(1 << 30)) return fail(GST_EINVAL, "n_slices*slice_mult = %lld exceeds 2^30", (long long)N);
+      if (N % (1LL << (depth - 1)) != 0)
+        return fail(GST_EINVAL, "2^(depth-1) = %ld does not divide the %lld slices of a thick element", 1L << (depth - 1), (long long)N);
     }
+  return GST_OK;
+}
+
+// Has a launch on this bunch failed since the last report?  Enqueues a 4-byte copy behind everything on `st`,
+// synchronises, and on failure clears the word (so that the bunch is usable again) and names the failure.
+gst_status sync_and_report(gst_bunch* b, cudaStream_t st) {
+  CUDA_TRY(cudaMemcpyAsync(b->h_err, b->d_err, sizeof(int), cudaMemcpyDeviceToHost, st));
+  CUDA_TRY(cudaStreamSynchronize(st));
+  if (*b->h_err != 0) {
+    CUDA_TRY(cudaMemsetAsync(b->d_err, 0, sizeof(int), st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return fail(GST_ECUDA, "%s: a hand-off between warp slots timed out (the chip made no progress); the particle arrays "
+                "of this bunch are undefined", b->last_kernel);
+  }
   return GST_OK;
 }
 
@@ -225,16 +250,11 @@ gst_status validate_track(const gst_lattice* lat, int64_t n_turns, int split, in
 
 extern "C" {
 
-const char* gst_last_error(void) { return g_err.c_str(); }
-
-gst_status gst_set_kernel_variant(gst_kernel_variant v) {
-  if (v != GST_KERNEL_FUSED && v != GST_KERNEL_PAIR && v != GST_KERNEL_FUSED_STATIC) return fail(GST_EINVAL, "unknown kernel variant %d", (int)v);
-  g_variant.store((int)v);
-  return GST_OK;
-}
+const char* gst_last_error(void) { return gst::g_err.c_str(); }
 
 gst_status gst_lattice_create(const gst_element* elems, size_t n, const gst_beam* beam, gst_lattice** out) {
   if (!elems || !beam || !out || n == 0) return fail(GST_EINVAL, "null argument or empty lattice");
+  if (n > (size_t)INT32_MAX) return fail(GST_EINVAL, "more than 2^31 - 1 elements");
   if (!(beam->gamma0 > 1.0) || !(beam->mass_eV > 0.0)) return fail(GST_EINVAL, "beam: need gamma0 > 1 and mass_eV > 0");
   for (size_t i = 0; i < n; ++i) {
     const gst_element& e = elems[i];
@@ -275,23 +295,50 @@ gst_status gst_lattice_create(const gst_element* elems, size_t n, const gst_beam
     lat->seq[i] = gst::seq_pack((uint32_t)k, e.type);
     if (e.type == GST_RFCAV) lat->cav_dEs.push_back(e.volt_eV * std::sin(e.phi_s));
   }
-  cudaError_t ce = cudaMalloc(&lat->d_seq, n * sizeof(uint32_t));
-  if (ce == cudaSuccess) ce = cudaMemcpy(lat->d_seq, lat->seq.data(), n * sizeof(uint32_t), cudaMemcpyHostToDevice);
+  // the sequence goes up through a pinned staging buffer on a stream of its own, complete when this call returns
+  // (a blocking copy from pageable memory may return before its DMA has landed, and streams made with
+  // cudaStreamNonBlocking -- torch's -- are not ordered behind the legacy stream)
+  cudaError_t ce = cudaGetDevice(&lat->device);
+  if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&lat->sms, cudaDevAttrMultiProcessorCount, lat->device);
+  uint32_t* h_seq = nullptr;
+  cudaStream_t up = nullptr;
+  if (ce == cudaSuccess) ce = cudaMalloc(&lat->d_seq, n * sizeof(uint32_t));
+  if (ce == cudaSuccess) ce = cudaMallocHost(&h_seq, n * sizeof(uint32_t));
+  if (ce == cudaSuccess) ce = cudaStreamCreateWithFlags(&up, cudaStreamNonBlocking);
+  if (ce == cudaSuccess) {
+    std::memcpy(h_seq, lat->seq.data(), n * sizeof(uint32_t));
+    ce = cudaMemcpyAsync(lat->d_seq, h_seq, n * sizeof(uint32_t), cudaMemcpyHostToDevice, up);
+  }
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(up);
+  if (up) cudaStreamDestroy(up);
+  if (h_seq) cudaFreeHost(h_seq);
   if (ce != cudaSuccess) {
     if (lat->d_seq) cudaFree(lat->d_seq);
     delete lat;
-    return fail(GST_ECUDA, "staging the element sequence: %s", cudaGetErrorString(ce));
+    return fail(ce == cudaErrorMemoryAllocation ? GST_ENOMEM : GST_ECUDA, "staging the element sequence: %s", cudaGetErrorString(ce));
   }
   *out = lat;
   return GST_OK;
 }
 
-void gst_lattice_destroy(gst_lattice* lat) {
-  if (!lat) return;
+static void drop_host_workspace(const gst_lattice* lat) {
   if (lat->ws_bunch) gst_bunch_destroy(lat->ws_bunch);
   if (lat->ws_state) cudaFree(lat->ws_state);
+  lat->ws_bunch = nullptr;
+  lat->ws_state = nullptr;
+  lat->ws_n = 0;
+}
+
+void gst_lattice_destroy(gst_lattice* lat) {
+  if (!lat) return;
+  DeviceGuard guard(lat->device);
+  drop_host_workspace(lat);
   if (lat->ws_stream) cudaStreamDestroy(lat->ws_stream);
-  for (auto& kv : lat->tables) cudaFree(kv.second.d_tab);
+  for (auto& kv : lat->tables) {
+    cudaEventDestroy(kv.second.ready);
+    cudaFree(kv.second.d_tab);
+    cudaFreeHost(kv.second.h_tab);
+  }
   cudaFree(lat->d_seq);
   delete lat;
 }
@@ -309,21 +356,33 @@ gst_status gst_bunch_init(double* x, double* px, double* y, double* py, double* 
   double* p[9] = {x, px, y, py, t, pt, sx, sy, ss};
   for (int i = 0; i < 9; ++i)
     if (!p[i] && n > 0) return fail(GST_EINVAL, "null state pointer %d", i);
+  int device = 0;
+  CUDA_TRY(cudaGetDevice(&device));
+  if (n > 0) {      // the bunch lives where its arrays live
+    cudaPointerAttributes at;
+    CUDA_TRY(cudaPointerGetAttributes(&at, x));
+    if (at.type == cudaMemoryTypeDevice) device = at.device;
+    else if (at.type != cudaMemoryTypeManaged) return fail(GST_EINVAL, "the state arrays must be device memory");
+  }
+  GUARD_DEVICE(device);
   gst_bunch* b = new (std::nothrow) gst_bunch;
   if (!b) return fail(GST_ENOMEM, "out of host memory");
   for (int i = 0; i < 9; ++i) b->p[i] = p[i];
   b->n = n;
+  b->device = device;
   cudaError_t ce = cudaMalloc(&b->d_lost, n > 0 ? n : 1);
   if (ce == cudaSuccess) ce = cudaMemset(b->d_lost, 0, n > 0 ? n : 1);
   if (ce == cudaSuccess) ce = cudaMalloc(&b->d_partials, sizeof(double) * gst::RED_MAX_BLOCKS * gst::RED_WIDTH);
   if (ce == cudaSuccess) ce = cudaMalloc(&b->d_result, sizeof(double) * 2 * gst::RED_WIDTH);
   if (ce == cudaSuccess) ce = cudaMallocHost(&b->h_result, sizeof(double) * 2 * gst::RED_WIDTH);
   const size_t n_chains = (n + 31) / 32 + 1;
-  // [sm scratch | chain flags], zeroed together before every rotating launch
-  if (ce == cudaSuccess) ce = cudaMalloc(&b->d_chain_flag, sizeof(int) * (n_chains + 2 * gst::CHAIN_MAX_SMID + 1));
+  // [scratch | chain flags], zeroed together before every rotating launch
+  if (ce == cudaSuccess) ce = cudaMalloc(&b->d_chain, sizeof(int) * (n_chains + gst::CHAIN_SCRATCH_INTS));
   if (ce == cudaSuccess) ce = cudaMalloc(&b->d_chain_E0, sizeof(double) * 2 * n_chains);
   if (ce == cudaSuccess) ce = cudaMalloc(&b->d_err, sizeof(int));
   if (ce == cudaSuccess) ce = cudaMemset(b->d_err, 0, sizeof(int));
+  if (ce == cudaSuccess) ce = cudaMallocHost(&b->h_err, sizeof(int));
+  if (ce == cudaSuccess) ce = cudaDeviceSynchronize();     // the memsets ran on the legacy stream: done before any launch
   if (ce != cudaSuccess) {
     gst_bunch_destroy(b);
     return fail(ce == cudaErrorMemoryAllocation ? GST_ENOMEM : GST_ECUDA, "gst_bunch_init: %s", cudaGetErrorString(ce));
@@ -334,13 +393,15 @@ gst_status gst_bunch_init(double* x, double* px, double* y, double* py, double* 
 
 void gst_bunch_destroy(gst_bunch* b) {
   if (!b) return;
+  DeviceGuard guard(b->device);
   if (b->d_lost) cudaFree(b->d_lost);
   if (b->d_partials) cudaFree(b->d_partials);
   if (b->d_result) cudaFree(b->d_result);
   if (b->h_result) cudaFreeHost(b->h_result);
-  if (b->d_chain_flag) cudaFree(b->d_chain_flag);
+  if (b->d_chain) cudaFree(b->d_chain);
   if (b->d_chain_E0) cudaFree(b->d_chain_E0);
   if (b->d_err) cudaFree(b->d_err);
+  if (b->h_err) cudaFreeHost(b->h_err);
   delete b;
 }
 
@@ -364,6 +425,18 @@ gst_status gst_bunch_set_reference(gst_bunch* b, const gst_beam* beam, int64_t t
   return GST_OK;
 }
 
+gst_status gst_bunch_set_launch(gst_bunch* b, gst_launch_mode mode) {
+  if (!b || (mode != GST_LAUNCH_AUTO && mode != GST_LAUNCH_STATIC)) return fail(GST_EINVAL, "null bunch or unknown launch mode %d", (int)mode);
+  b->launch_mode = mode;
+  return GST_OK;
+}
+
+gst_status gst_diag_chain_poll_limit(gst_bunch* b, int64_t polls) {
+  if (!b || polls < 0) return fail(GST_EINVAL, "null bunch or negative poll count");
+  b->poll_limit_override = -(long long)polls;       // negative = absolute count (track_chain_kernel.cuh)
+  return GST_OK;
+}
+
 // depth_code >= 1: trapezoid/Romberg scheme of that depth; 0 / -1: mid-slice PWC (half-slice / DKSKD ordering),
 // for which the element table is derived for 2 n_slices half slices
 static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, gst_split split, int n_slices,
@@ -372,6 +445,9 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   gst_status vs = validate_track(lat, n_turns, (int)split, n_slices, depth_code >= 1 ? depth_code : 1);
   if (vs != GST_OK) return vs;
   if (depth_code < 1 && (int)split > 2) return fail(GST_EINVAL, "gst_track_pwc takes the second-order splits only");
+  if (b->n > 0 && b->device != lat->device)
+    return fail(GST_EINVAL, "the bunch lives on device %d, the lattice on device %d", b->device, lat->device);
+  GUARD_DEVICE(lat->device);
   const int romberg_depth = depth_code;
   const int table_slices = depth_code >= 1 ? n_slices : 2 * n_slices;
   if (!b->have_ref) {
@@ -381,45 +457,46 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
     b->have_ref = true;
   }
   if (b->n == 0 || n_turns == 0) return GST_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
   const gst::DevElem* d_tab = nullptr;
-  gst_status ts = get_table(lat, table_slices, &d_tab);
+  gst_status ts = get_table(lat, table_slices, st, &d_tab);
   if (ts != GST_OK) return ts;
-  gst::TrackArgs a;
+  gst::LaunchRequest rq;
+  gst::TrackArgs& a = rq.args;
   for (int i = 0; i < 9; ++i) a.p[i] = b->p[i];
   a.lost = b->d_lost;
   a.tab = d_tab;
   a.seq = lat->d_seq;
   a.n_unique = (int)lat->uniq.size();
   a.n_seq = (int)lat->seq.size();
+  a.use_smem_seq = 0;
+  a.use_smem_tab = 0;
   a.n = (long long)b->n;
   a.n_turns = n_turns;
   a.E0 = b->E0;
   a.E0lo = b->E0lo;
   a.mass = b->mass;
   a.G = lat->beam.G;
-  size_t tab_bytes = lat->uniq.size() * sizeof(gst::DevElem);
-  size_t seq_bytes = (lat->seq.size() * sizeof(uint32_t) + 15) & ~size_t(15);
-  const bool pair = g_variant.load() == GST_KERNEL_PAIR;
-  gst::ChainLaunch chain_req;
-  chain_req.args.sm_scratch = b->d_chain_flag;
-  chain_req.args.flag = b->d_chain_flag + 2 * gst::CHAIN_MAX_SMID + 1;
-  chain_req.args.E0 = b->d_chain_E0;
-  chain_req.args.err = b->d_err;
-  chain_req.steps_per_turn = gst_lattice_steps_per_turn(lat, table_slices);
-  gst::ChainLaunch* chain = g_variant.load() == GST_KERNEL_FUSED ? &chain_req : nullptr;
-  a.use_smem_seq = 0;
-  a.use_smem_tab = 0;
-  cudaStream_t st = (cudaStream_t)cuda_stream;
+  a.err = b->d_err;
+  rq.tab_bytes = lat->uniq.size() * sizeof(gst::DevElem);
+  rq.seq_bytes = (lat->seq.size() * sizeof(uint32_t) + 15) & ~size_t(15);
+  rq.steps_per_turn = gst_lattice_steps_per_turn(lat, table_slices);
+  rq.sms = lat->sms;
+  rq.allow_chain = b->launch_mode == GST_LAUNCH_AUTO;
+  rq.chain.scratch = b->d_chain;
+  rq.chain.flag = b->d_chain + gst::CHAIN_SCRATCH_INTS;
+  rq.chain.E0 = b->d_chain_E0;
+  rq.chain.err = b->d_err;
+  rq.poll_limit_override = b->poll_limit_override;
   cudaError_t ce;
   const int order = (int)split >= 3 ? 4 : 2;
   switch ((int)split % 3) {
-    case 0: ce = gst::launch_split_dk(order, romberg_depth, a, tab_bytes, seq_bytes, pair, st, chain); break;
-    case 1: ce = gst::launch_split_bk(order, romberg_depth, a, tab_bytes, seq_bytes, pair, st, chain); break;
-    default: ce = gst::launch_split_mk(order, romberg_depth, a, tab_bytes, seq_bytes, pair, st, chain); break;
+    case 0: ce = gst::launch_split_dk(order, romberg_depth, rq, st); break;
+    case 1: ce = gst::launch_split_bk(order, romberg_depth, rq, st); break;
+    default: ce = gst::launch_split_mk(order, romberg_depth, rq, st); break;
   }
   if (ce != cudaSuccess) return fail(GST_ECUDA, "track launch: %s", cudaGetErrorString(ce));
-  b->last_kernel = pair && romberg_depth >= 1 && (int)split < 3 ? "track_pair_kernel"
-                   : (chain_req.taken ? "track_chain_kernel" : "track_kernel");
+  b->last_kernel = rq.kernel;
   // host-side bookkeeping of the reference energy: the same IEEE operations the kernel performs
   for (int64_t t = 0; t < n_turns; ++t)
     for (double dEs : lat->cav_dEs)
@@ -440,6 +517,12 @@ gst_status gst_track_pwc(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, 
   return track_impl(b, lat, n_turns, split, n_slices, order == GST_PWC_HALF_SLICE ? 0 : -1, cuda_stream);
 }
 
+gst_status gst_bunch_status(gst_bunch* b, void* cuda_stream) {
+  if (!b) return fail(GST_EINVAL, "null bunch");
+  GUARD_DEVICE(b->device);
+  return sync_and_report(b, (cudaStream_t)cuda_stream);
+}
+
 static gst_status run_moments(gst_bunch* b, cudaStream_t st, bool second) {
   int blocks = (int)((b->n + gst::RED_BLOCK - 1) / gst::RED_BLOCK);
   if (blocks > gst::RED_MAX_BLOCKS) blocks = gst::RED_MAX_BLOCKS;
@@ -458,15 +541,12 @@ static gst_status run_moments(gst_bunch* b, cudaStream_t st, bool second) {
   }
   CUDA_TRY(cudaGetLastError());
   CUDA_TRY(cudaMemcpyAsync(b->h_result, b->d_result, sizeof(double) * 2 * gst::RED_WIDTH, cudaMemcpyDeviceToHost, st));
-  int err = 0;
-  CUDA_TRY(cudaMemcpyAsync(&err, b->d_err, sizeof(int), cudaMemcpyDeviceToHost, st));
-  CUDA_TRY(cudaStreamSynchronize(st));
-  if (err) return fail(GST_ECUDA, "track_chain_kernel: a chain handoff timed out (not every warp slot was resident)");
-  return GST_OK;
+  return sync_and_report(b, st);
 }
 
 gst_status gst_polarization(gst_bunch* b, void* cuda_stream, double out[4], int64_t* out_lost) {
   if (!b || !out) return fail(GST_EINVAL, "null argument");
+  GUARD_DEVICE(b->device);
   gst_status s = run_moments(b, (cudaStream_t)cuda_stream, false);
   if (s != GST_OK) return s;
   const double* r = b->h_result;   // {sum Sx, Sy, Ss, alive, sum X, Px, Y, Py}
@@ -480,6 +560,7 @@ gst_status gst_polarization(gst_bunch* b, void* cuda_stream, double out[4], int6
 
 gst_status gst_emittance(gst_bunch* b, void* cuda_stream, double out_exy[2]) {
   if (!b || !out_exy) return fail(GST_EINVAL, "null argument");
+  GUARD_DEVICE(b->device);
   gst_status s = run_moments(b, (cudaStream_t)cuda_stream, true);
   if (s != GST_OK) return s;
   const double* r = b->h_result;
@@ -496,10 +577,10 @@ gst_status gst_emittance(gst_bunch* b, void* cuda_stream, double out_exy[2]) {
 
 gst_status gst_bunch_lost(gst_bunch* b, void* cuda_stream, uint8_t* host_out) {
   if (!b || !host_out) return fail(GST_EINVAL, "null argument");
+  GUARD_DEVICE(b->device);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   if (b->n) CUDA_TRY(cudaMemcpyAsync(host_out, b->d_lost, b->n, cudaMemcpyDeviceToHost, st));
-  CUDA_TRY(cudaStreamSynchronize(st));
-  return GST_OK;
+  return sync_and_report(b, st);
 }
 
 gst_status gst_track_host(const gst_lattice* lat, double* const host_state[9], size_t n, int64_t n_turns,
@@ -507,18 +588,16 @@ gst_status gst_track_host(const gst_lattice* lat, double* const host_state[9], s
   if (!lat || !host_state || !out_pol) return fail(GST_EINVAL, "null argument");
   gst_status vs = validate_track(lat, n_turns, (int)split, n_slices, romberg_depth);
   if (vs != GST_OK) return vs;
+  GUARD_DEVICE(lat->device);
   std::lock_guard<std::mutex> lk(lat->mu_host);
-  if (!lat->ws_stream) CUDA_TRY(cudaStreamCreate(&lat->ws_stream));
+  if (!lat->ws_stream) CUDA_TRY(cudaStreamCreateWithFlags(&lat->ws_stream, cudaStreamNonBlocking));
   if (!lat->ws_bunch || lat->ws_n != n) {          // (re)build the workspace for this bunch size
-    if (lat->ws_bunch) gst_bunch_destroy(lat->ws_bunch);
-    if (lat->ws_state) cudaFree(lat->ws_state);
-    lat->ws_bunch = nullptr;
-    lat->ws_state = nullptr;
+    drop_host_workspace(lat);
     CUDA_TRY(cudaMalloc(&lat->ws_state, sizeof(double) * 9 * (n ? n : 1)));
     double* d0 = lat->ws_state;
     gst_status bs = gst_bunch_init(d0, d0 + n, d0 + 2 * n, d0 + 3 * n, d0 + 4 * n, d0 + 5 * n, d0 + 6 * n, d0 + 7 * n,
                                    d0 + 8 * n, n, &lat->ws_bunch);
-    if (bs != GST_OK) return bs;
+    if (bs != GST_OK) { drop_host_workspace(lat); return bs; }
     lat->ws_n = n;
   }
   double* d = lat->ws_state;
@@ -532,67 +611,20 @@ gst_status gst_track_host(const gst_lattice* lat, double* const host_state[9], s
     ce = cudaMemcpyAsync(d + i * n, host_state[i], sizeof(double) * n, cudaMemcpyHostToDevice, st);
   if (ce != cudaSuccess) s = fail(GST_ECUDA, "H2D: %s", cudaGetErrorString(ce));
   if (s == GST_OK) s = gst_track(b, lat, n_turns, split, n_slices, romberg_depth, st);
-  if (s == GST_OK) s = gst_polarization(b, st, out_pol, out_lost);
+  if (s == GST_OK) s = gst_polarization(b, st, out_pol, out_lost);     // synchronises and reports a failed launch
   if (s == GST_OK) {
     for (int i = 0; i < 9 && ce == cudaSuccess; ++i)
       ce = cudaMemcpyAsync(host_state[i], d + i * n, sizeof(double) * n, cudaMemcpyDeviceToHost, st);
     if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
     if (ce != cudaSuccess) s = fail(GST_ECUDA, "D2H: %s", cudaGetErrorString(ce));
   }
+  if (s != GST_OK) {                                // nothing of a failed call is kept for the next one
+    const std::string msg = gst::g_err;
+    cudaStreamSynchronize(st);
+    drop_host_workspace(lat);
+    gst::g_err = msg;
+  }
   return s;
 }
-
-gst_status gst_selftest_math(double out[2]) {
-  if (!out) return fail(GST_EINVAL, "null argument");
-  unsigned long long* d = nullptr;
-  CUDA_TRY(cudaMalloc(&d, 16));
-  CUDA_TRY(cudaMemset(d, 0, 16));
-  math_selftest_kernel<<<296, 256>>>(d, 1 << 24);
-  unsigned long long h[2];
-  cudaError_t ce = cudaMemcpy(h, d, 16, cudaMemcpyDeviceToHost);
-  cudaFree(d);
-  if (ce != cudaSuccess) return fail(GST_ECUDA, "selftest: %s", cudaGetErrorString(ce));
-  for (int k = 0; k < 2; ++k) {
-    double v;
-    std::memcpy(&v, &h[k], 8);
-    out[k] = v / 1.1102230246251565e-16;      // in units of 2^-53
-  }
-  return GST_OK;
-}
-
-static gst_status fp64_peak_impl(bool three_registers, double* out_tflops, double* out_ms) {
-  if (!out_tflops) return fail(GST_EINVAL, "null argument");
-  int dev = 0, sms = 0;
-  CUDA_TRY(cudaGetDevice(&dev));
-  CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  double* d_out = nullptr;
-  CUDA_TRY(cudaMalloc(&d_out, sizeof(double) * sms * 8 * gst::PEAK_BLOCK));
-  cudaEvent_t e0, e1;
-  CUDA_TRY(cudaEventCreate(&e0));
-  CUDA_TRY(cudaEventCreate(&e1));
-  const int iters = 1 << 14;
-  float best = 1e30f;
-  for (int rep = 0; rep < 6; ++rep) {
-    cudaEventRecord(e0);
-    if (three_registers) gst::dfma_rrr_kernel<<<sms * 8, gst::PEAK_BLOCK>>>(d_out, iters, 1.0 + 1e-9 * rep);
-    else gst::dfma_peak_kernel<<<sms * 8, gst::PEAK_BLOCK>>>(d_out, iters, 1.0 + 1e-9 * rep);
-    cudaEventRecord(e1);
-    CUDA_TRY(cudaEventSynchronize(e1));
-    float ms = 0;
-    cudaEventElapsedTime(&ms, e0, e1);
-    if (rep > 0 && ms < best) best = ms;
-  }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  cudaFree(d_out);
-  CUDA_TRY(cudaGetLastError());
-  double flops = 2.0 * gst::PEAK_CHAINS * (double)iters * gst::PEAK_UNROLL * (double)sms * 8 * gst::PEAK_BLOCK;
-  *out_tflops = flops / (best * 1e-3) / 1e12;
-  if (out_ms) *out_ms = best;
-  return GST_OK;
-}
-
-gst_status gst_fp64_peak(double* out_tflops, double* out_ms) { return fp64_peak_impl(false, out_tflops, out_ms); }
-gst_status gst_fp64_peak_rrr(double* out_tflops, double* out_ms) { return fp64_peak_impl(true, out_tflops, out_ms); }
 
 }  // extern "C"

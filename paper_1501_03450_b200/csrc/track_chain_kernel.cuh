@@ -11,19 +11,24 @@
 //   M < S : in every round S - M slots find that their chain's previous chunk is still being computed and
 //           wait; because S is not a multiple of M these idle slots wander over the chip, so every
 //           sub-partition carries the same load over the launch.
-// Nothing is barrier-synchronised: chunk k of a chain may start as soon as its chunk k-1 is stored, which a
-// per-chain flag (release / acquire at GPU scope) announces; the state (72 B per particle) and the chain's
+// Nothing but the start is barrier-synchronised: chunk k of a chain may start as soon as its chunk k-1 is stored,
+// which a per-chain flag (release / acquire at GPU scope) announces; the state (72 B per particle) and the chain's
 // reference energy travel through global memory, bypassing the incoherent L1.
 //
-// Which slots idle together matters: the slots are numbered v = (warp index on its SM) * n_sm + (rank of the SM), from
-// %smid and two atomics at kernel start, so that slots that are neighbours in v -- the ones that idle together -- sit
-// on different SMs, whatever order the hardware places the blocks in (with the block index as slot number a
-// cooperative launch was 4 % slower than a plain one).
+// Which slots idle together matters: neighbours in the slot number v -- the ones that idle together -- must sit on
+// different SMs, whatever order the hardware places the blocks in (with the block index as slot number a cooperative
+// launch was 4 % slower than a plain one).  Every block therefore registers on its SM (%smid: its index l among the
+// blocks there, the SM's rank by first arrival), all blocks meet once at a start barrier (the launch is cooperative,
+// so they are co-resident), and then each computes its number from the final per-SM counts:
+//   v = 2 * #{blocks with index < l} + w * n_l + #{SMs that hold more than l blocks and rank below this one's},
+// w = warp in the block, n_l = SMs holding more than l blocks.  This is a bijection onto 0..S-1 for ANY distribution
+// of the blocks over the SMs (a cooperative launch guarantees co-residency, not an even spread), and SM-interleaved.
 //
 // Correct by induction on p (a position waits only for position p - M, which its slot reaches earlier in its own
-// order), provided every slot is resident: the host launches the occupancy-sized grid cooperatively and falls
-// back to track_kernel otherwise.  Bounded waits guard against a hang.
-// The arithmetic is the fused kernel's: results are bit-identical.
+// order), provided every slot is resident: the host launches the grid cooperatively and falls back to track_kernel
+// when that is refused.  Waits are bounded by PROGRESS: a waiting warp gives up when no chunk anywhere on the chip
+// has completed for `poll_limit` polls (scaled by the host with the length of a chunk), sets the bunch's error word
+// and leaves; everybody else follows.  The arithmetic is the fused kernel's: results are bit-identical.
 #pragma once
 #include "track_kernel.cuh"
 
@@ -33,94 +38,134 @@
 
 namespace gst {
 
-struct ChainArgs {
-  int n_chains;        // ceil(n / 32)
-  int chunk_turns;     // turns per chunk
-  int n_sm;            // SMs in use = gridDim.x / blocks per SM
-  int* sm_scratch;     // [2 * CHAIN_MAX_SMID + 1] blocks arrived per SM, rank + 1 per SM, SMs ranked; zeroed with flag[]
-  int* flag;           // [n_chains] chunks completed, zeroed before the launch
-  double* E0;          // [2 n_chains] reference energy after the chain's last chunk: E0 at [c], E0lo at [n_chains + c]
-  int* err;            // set to 1 when a wait times out
-};
-
 constexpr int CHAIN_MAX_SMID = 512;
+// layout of the per-bunch int scratch, zeroed (together with the chain flags behind it) before every rotating launch
+constexpr int CHAIN_COUNT = 0;                        // [CHAIN_MAX_SMID] blocks registered per SM
+constexpr int CHAIN_RANK = CHAIN_MAX_SMID;            // [CHAIN_MAX_SMID] rank + 1 of the SM by first arrival
+constexpr int CHAIN_NRANKED = 2 * CHAIN_MAX_SMID;     // SMs ranked so far
+constexpr int CHAIN_ARRIVED = 2 * CHAIN_MAX_SMID + 1; // blocks at the start barrier
+constexpr int CHAIN_PROGRESS = 2 * CHAIN_MAX_SMID + 2;// chunks completed, all chains
+constexpr int CHAIN_SCRATCH_INTS = 2 * CHAIN_MAX_SMID + 4;
+
+struct ChainArgs {
+  int n_chains;          // ceil(n / 32)
+  int chunk_turns;       // turns per chunk
+  int* scratch;          // [CHAIN_SCRATCH_INTS], see above
+  int* flag;             // [n_chains] chunks completed per chain
+  double* E0;            // [2 n_chains] reference energy after the chain's last chunk: E0 at [c], E0lo at [n_chains + c]
+  int* err;              // the bunch's error word (sticky until the host reports it)
+  long long poll_limit;  // > 0: give up after this many polls WITHOUT PROGRESS anywhere; < 0: after -poll_limit polls
+                         // whatever happens elsewhere (fault injection, include/gst_diag.h)
+};
 
 __device__ __forceinline__ int ld_acquire(const int* p) {
   int v;
   asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
+__device__ __forceinline__ int ld_relaxed(const int* p) {
+  int v;
+  asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
 __device__ __forceinline__ void st_release(int* p, int v) {
   asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// Number this block's first warp slot (see the header).  Returns -1 when the start barrier timed out.
+__device__ __forceinline__ long long chain_slot_of_block(const ChainArgs& ch, int warps_per_block) {
+  __shared__ int s_l, s_rank, s_part[3];
+  int* sc = ch.scratch;
+  if (threadIdx.x == 0) {
+    unsigned sm;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
+    sm %= CHAIN_MAX_SMID;
+    const int l = atomicAdd(sc + CHAIN_COUNT + sm, 1);                    // this block's index on its SM
+    if (l == 0) st_release(sc + CHAIN_RANK + sm, atomicAdd(sc + CHAIN_NRANKED, 1) + 1);
+    __threadfence();
+    atomicAdd(sc + CHAIN_ARRIVED, 1);
+    int tries = 0;
+    bool ok = true;
+    while (ld_acquire(sc + CHAIN_ARRIVED) < (int)gridDim.x) {             // start barrier: the counts are final after it
+      __nanosleep(128);
+      if (++tries > (1 << 22) || ld_relaxed(ch.err) != 0) { ok = false; break; }
+    }
+    s_l = ok ? l : -1;
+    s_rank = ok ? ld_acquire(sc + CHAIN_RANK + sm) - 1 : -1;
+    s_part[0] = s_part[1] = s_part[2] = 0;
+  }
+  __syncthreads();
+  const int l = s_l, rank = s_rank;
+  if (l < 0 || rank < 0) return -1;
+  // blocks with a smaller index, SMs on this level, SMs on this level ranked below this one: summed over the SM ids
+  int below = 0, level = 0, before = 0;
+  for (int s = threadIdx.x; s < CHAIN_MAX_SMID; s += blockDim.x) {
+    const int c = ld_relaxed(sc + CHAIN_COUNT + s);
+    if (c == 0) continue;
+    below += c < l ? c : l;
+    if (c > l) {
+      ++level;
+      if (ld_relaxed(sc + CHAIN_RANK + s) - 1 < rank) ++before;
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    below += __shfl_down_sync(0xffffffffu, below, o);
+    level += __shfl_down_sync(0xffffffffu, level, o);
+    before += __shfl_down_sync(0xffffffffu, before, o);
+  }
+  if ((threadIdx.x & 31) == 0) {
+    atomicAdd(&s_part[0], below);
+    atomicAdd(&s_part[1], level);
+    atomicAdd(&s_part[2], before);
+  }
+  __syncthreads();
+  // warp w of this block: slot = warps_per_block * below + w * level + before
+  return ((long long)s_part[1] << 32) | (unsigned)(warps_per_block * s_part[0] + s_part[2]);
 }
 
 template <int SPLIT, int DEPTH, int ORDER>
 __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_chain_kernel(const TrackArgs a, const ChainArgs ch) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  // a0: stage the unique-element table and the sequence into shared memory, each when it fits
-  const DevElem* tab = a.tab;
-  const uint32_t* seq = a.seq;
-  {
-    size_t off = 0;
-    if (a.use_smem_tab) {
-      const int nw = a.n_unique * (int)(sizeof(DevElem) / sizeof(double));
-      const double* src = reinterpret_cast<const double*>(a.tab);
-      double* dst = reinterpret_cast<double*>(smem_raw);
-      for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
-      tab = reinterpret_cast<const DevElem*>(smem_raw);
-      off = (size_t)a.n_unique * sizeof(DevElem);
-    }
-    if (a.use_smem_seq) {
-      uint32_t* sseq = reinterpret_cast<uint32_t*>(smem_raw + off);
-      for (int i = threadIdx.x; i < a.n_seq; i += blockDim.x) sseq[i] = a.seq[i];
-      seq = sseq;
-    }
-    __syncthreads();
-  }
+  const DevElem* tab;
+  const uint32_t* seq;
+  stage_lattice(a, smem_raw, tab, seq);
+  if (*a.err != 0) return;                               // an earlier launch on this bunch failed: leave everything (gst.h)
   const int lane = threadIdx.x & 31;
   const long long slots = (long long)gridDim.x * (TRACK_BLOCK / 32);
-  __shared__ int s_local, s_rank;
-  if (threadIdx.x == 0) {      // number the slots SM-interleaved (see the header)
-    unsigned sm;
-    asm volatile("mov.u32 %0, %%smid;" : "=r"(sm));
-    sm %= CHAIN_MAX_SMID;
-    const int l = atomicAdd(ch.sm_scratch + sm, 1);                       // this block's index on its SM
-    int rank;
-    if (l == 0) {
-      rank = atomicAdd(ch.sm_scratch + 2 * CHAIN_MAX_SMID, 1);
-      st_release(ch.sm_scratch + CHAIN_MAX_SMID + sm, rank + 1);
-    } else {
-      int tries = 0;
-      while ((rank = ld_acquire(ch.sm_scratch + CHAIN_MAX_SMID + sm)) == 0) {
-        __nanosleep(64);
-        if (++tries > (1 << 24)) { *ch.err = 1; break; }
-      }
-      rank -= 1;
-    }
-    s_local = l;
-    s_rank = rank;
-  }
-  __syncthreads();
-  if (s_rank < 0 || s_rank >= ch.n_sm || s_local * (TRACK_BLOCK / 32) >= slots / ch.n_sm) {   // not the placement assumed
-    if (threadIdx.x == 0) *ch.err = 1;
+  const long long packed = chain_slot_of_block(ch, TRACK_BLOCK / 32);
+  if (packed < 0) {
+    if (threadIdx.x == 0) atomicExch(ch.err, 1);
     return;
   }
-  const long long slot = (long long)(s_local * (TRACK_BLOCK / 32) + (threadIdx.x >> 5)) * ch.n_sm + s_rank;
+  const long long slot = (long long)(unsigned)(packed & 0xffffffffLL) + (long long)(threadIdx.x >> 5) * (packed >> 32);
   const long long n_chunks = (a.n_turns + ch.chunk_turns - 1) / ch.chunk_turns;
   const long long M = ch.n_chains;
   const long long total = n_chunks * M;
+  int* progress = ch.scratch + CHAIN_PROGRESS;
   for (long long p = slot; p < total; p += slots) {
     const long long k = p / M, c = p - k * M;             // chunk k of chain c
     if (k > 0) {                                          // chunk k-1 of this chain is stored
       // a chunk runs for milliseconds: poll with a back-off of up to GST_CHAIN_POLL_NS, so that the warps that wait
       // (320 of the 2368 slots at any time for 65 536 particles) do not take issue slots from the ones that work
-      int tries = 0;
+      long long polls = 0, idle = 0;
+      int seen = 0;
       unsigned ns = 256;
 #pragma unroll 1
       while (ld_acquire(ch.flag + c) < (int)k) {
         __nanosleep(ns);
         if (ns < GST_CHAIN_POLL_NS) ns *= 2;
-        if (++tries > (1 << 21)) { *ch.err = 1; return; }     // ~20 s: no chunk takes that long
+        ++polls;
+        if ((polls & 15) == 0 || ch.poll_limit < 0) {     // every 16th poll: has anything on the chip moved?
+          const int now = ld_relaxed(progress);
+          idle = now != seen ? 0 : idle + 16;
+          seen = now;
+          const bool out_of_time = ch.poll_limit > 0 ? idle > ch.poll_limit : polls > -ch.poll_limit;
+          if (out_of_time || ld_relaxed(ch.err) != 0) {
+            atomicExch(ch.err, 1);
+            return;
+          }
+        }
       }
     }
     const long long j = c * 32 + lane;
@@ -138,25 +183,10 @@ __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_chain_ker
     ref.E0lo = k == 0 ? a.E0lo : __ldcg(ch.E0 + ch.n_chains + c);
     PCon pc;
     pcon_set(pc, z.Pt, ref, a.G);
-    bool lost = false;
     typename SpinPolicy<DEPTH, SPLIT>::type spin(z);
     const long long t0 = k * ch.chunk_turns;
     const long long t1 = t0 + ch.chunk_turns < a.n_turns ? t0 + ch.chunk_turns : a.n_turns;
-    uint32_t nxt = seq[0];
-    for (long long turn = t0; turn < t1; ++turn) {
-#pragma unroll 1
-      for (int ie = 0; ie < a.n_seq; ++ie) {
-        const uint32_t cur = nxt;
-        nxt = seq[ie + 1 < a.n_seq ? ie + 1 : 0];
-        const DevElem& e = tab[cur >> 8];
-        const bool ok = element_step<SPLIT, ORDER>((int)(cur & 0xffu), z, e, pc, ref, a.G, spin);
-        if (!ok) {
-          lost = true;
-          z.X = z.Px = z.Y = z.Py = z.T = z.Pt = 0.0;
-          pcon_set(pc, 0.0, ref, a.G);
-        }
-      }
-    }
+    const bool lost = track_turns<SPLIT, ORDER>(z, ref, pc, spin, t0, t1, tab, seq, a.n_seq, a.G);
     if (valid) {
       if (lost) {
         a.lost[j] = 1;
@@ -172,7 +202,10 @@ __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_chain_ker
     }
     __threadfence();
     __syncwarp();
-    if (lane == 0) st_release(ch.flag + c, (int)k + 1);
+    if (lane == 0) {
+      st_release(ch.flag + c, (int)k + 1);
+      atomicAdd(progress, 1);
+    }
   }
 }
 

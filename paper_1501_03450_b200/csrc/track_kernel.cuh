@@ -87,6 +87,8 @@ struct TrackArgs {
   long long n;
   long long n_turns;
   double E0, E0lo, mass, G;   // reference energy = E0 + E0lo (compensated sum of the cavity gains)
+  const int* err;           // the bunch's error word: non-zero = an earlier launch on this bunch failed and nobody has been
+                            // told yet; the kernel then leaves everything as it is (include/gst.h, "Errors")
 };
 
 // One sequence entry carries the element type next to the table index, so that the per-element dispatch
@@ -359,8 +361,8 @@ __device__ __forceinline__ bool drift(State& z, double L, PCon& c, const Ref& r)
 // current point; the spin policy's run() drives it through the N slices with the spin work software-pipelined.
 // ---------------------------------------------------------------------------------------------
 // The spin side of a thick element is a policy object with one method, run(stepper, N, ds):
-//   FusedSpin<DEPTH>  -- this thread folds every edge into its own level products (one thread per particle)
-//   PushSpin          -- track_pair_kernel.cuh: the edge rotation vectors go to a partner thread through shared memory
+//   FusedSpin<DEPTH>  -- the trapezoid / Romberg scheme (38)(39): every edge is folded into DEPTH level products
+//   MidSpin<KIND>     -- the mid-slice comparison integrators (37)
 // ROLLED: the matrix-kick kernels take the edges one per iteration with the level membership tested at run time
 // (uniform branches).  Their two-edge loop body would be 6.4 kB for the quadrupole (160 fp64 instructions per
 // slice), more than the 6 kB L0 instruction cache: rolled, matrix-kick runs 12-18 % faster (bends included), while
@@ -1122,32 +1124,62 @@ constexpr int TRACK_MIN_BLOCKS = 8;
 // faster; every other instantiation is equal or slightly slower that way (profiles/r01_notes.md).
 __host__ __device__ constexpr int track_min_blocks(int split, int order) { return (split == SPLIT_MK && order == 4) ? 6 : TRACK_MIN_BLOCKS; }
 
+// a0: stage the unique-element table and the sequence into shared memory, each when it fits (host plan: track_launch.cuh)
+__device__ __forceinline__ void stage_lattice(const TrackArgs& a, unsigned char* smem_raw, const DevElem*& tab,
+                                              const uint32_t*& seq) {
+  tab = a.tab;
+  seq = a.seq;
+  size_t off = 0;
+  if (a.use_smem_tab) {
+    const int nw = a.n_unique * (int)(sizeof(DevElem) / sizeof(double));
+    const double* src = reinterpret_cast<const double*>(a.tab);
+    double* dst = reinterpret_cast<double*>(smem_raw);
+    for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
+    tab = reinterpret_cast<const DevElem*>(smem_raw);
+    off = (size_t)a.n_unique * sizeof(DevElem);
+  }
+  if (a.use_smem_seq) {
+    uint32_t* sseq = reinterpret_cast<uint32_t*>(smem_raw + off);
+    for (int i = threadIdx.x; i < a.n_seq; i += blockDim.x) sseq[i] = a.seq[i];
+    seq = sseq;
+  }
+  __syncthreads();
+}
+
+// Turns [t0, t1) of the ring for one particle.  The turn and element loops run to the end for every thread, so
+// that their counters, the sequence loads and the type dispatch are warp-uniform (uniform registers, no divergence
+// bookkeeping); a particle that is lost (A15) goes on with the reference orbit and nothing of it is stored (R6).
+template <int SPLIT, int ORDER, class Spin>
+__device__ __forceinline__ bool track_turns(State& z, Ref& ref, PCon& pc, Spin& spin, long long t0, long long t1,
+                                            const DevElem* tab, const uint32_t* seq, int n_seq, double G) {
+  bool lost = false;
+  uint32_t nxt = seq[0];
+  for (long long turn = t0; turn < t1; ++turn) {
+#pragma unroll 1
+    for (int ie = 0; ie < n_seq; ++ie) {
+      const uint32_t cur = nxt;
+      nxt = seq[ie + 1 < n_seq ? ie + 1 : 0];          // next element's entry, one element ahead
+      const DevElem& e = tab[cur >> 8];
+      const bool ok = element_step<SPLIT, ORDER>((int)(cur & 0xffu), z, e, pc, ref, G, spin);
+      if (!ok) {
+        lost = true;
+        z.X = z.Px = z.Y = z.Py = z.T = z.Pt = 0.0;
+        pcon_set(pc, 0.0, ref, G);
+      }
+    }
+  }
+  return lost;
+}
+
 template <int SPLIT, int DEPTH, int ORDER>
 __global__ void __launch_bounds__(TRACK_BLOCK, track_min_blocks(SPLIT, ORDER)) track_kernel(const TrackArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  // a0: stage the unique-element table and the sequence into shared memory, each when it fits
-  const DevElem* tab = a.tab;
-  const uint32_t* seq = a.seq;
-  {
-    size_t off = 0;
-    if (a.use_smem_tab) {
-      const int nw = a.n_unique * (int)(sizeof(DevElem) / sizeof(double));
-      const double* src = reinterpret_cast<const double*>(a.tab);
-      double* dst = reinterpret_cast<double*>(smem_raw);
-      for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
-      tab = reinterpret_cast<const DevElem*>(smem_raw);
-      off = (size_t)a.n_unique * sizeof(DevElem);
-    }
-    if (a.use_smem_seq) {
-      uint32_t* sseq = reinterpret_cast<uint32_t*>(smem_raw + off);
-      for (int i = threadIdx.x; i < a.n_seq; i += blockDim.x) sseq[i] = a.seq[i];
-      seq = sseq;
-    }
-    __syncthreads();
-  }
+  const DevElem* tab;
+  const uint32_t* seq;
+  stage_lattice(a, smem_raw, tab, seq);
   const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= a.n) return;
-  if (a.lost[j]) return;
+  if (*a.err != 0 || a.lost[j]) return;
   State z;
   z.X = a.p[0][j]; z.Px = a.p[1][j]; z.Y = a.p[2][j]; z.Py = a.p[3][j]; z.T = a.p[4][j]; z.Pt = a.p[5][j];
   z.Sx = a.p[6][j]; z.Sy = a.p[7][j]; z.Ss = a.p[8][j];
@@ -1156,26 +1188,8 @@ __global__ void __launch_bounds__(TRACK_BLOCK, track_min_blocks(SPLIT, ORDER)) t
   ref.E0lo = a.E0lo;
   PCon pc;
   pcon_set(pc, z.Pt, ref, a.G);
-  // The turn and element loops run to the end for every thread, so that their counters, the sequence
-  // loads and the type dispatch are warp-uniform (uniform registers, no divergence bookkeeping); a
-  // particle that is lost (A15) goes on with the reference orbit and nothing of it is stored.
-  bool lost = false;
   typename SpinPolicy<DEPTH, SPLIT>::type spin(z);
-  uint32_t nxt = seq[0];
-  for (long long turn = 0; turn < a.n_turns; ++turn) {
-#pragma unroll 1
-    for (int ie = 0; ie < a.n_seq; ++ie) {
-      const uint32_t cur = nxt;
-      nxt = seq[ie + 1 < a.n_seq ? ie + 1 : 0];          // next element's entry, one element ahead
-      const DevElem& e = tab[cur >> 8];
-      const bool ok = element_step<SPLIT, ORDER>((int)(cur & 0xffu), z, e, pc, ref, a.G, spin);
-      if (!ok) {
-        lost = true;
-        z.X = z.Px = z.Y = z.Py = z.T = z.Pt = 0.0;
-        pcon_set(pc, 0.0, ref, a.G);
-      }
-    }
-  }
+  const bool lost = track_turns<SPLIT, ORDER>(z, ref, pc, spin, 0, a.n_turns, tab, seq, a.n_seq, a.G);
   if (lost) { a.lost[j] = 1; return; }
   a.p[0][j] = z.X; a.p[1][j] = z.Px; a.p[2][j] = z.Y; a.p[3][j] = z.Py; a.p[4][j] = z.T; a.p[5][j] = z.Pt;
   a.p[6][j] = z.Sx; a.p[7][j] = z.Sy; a.p[8][j] = z.Ss;

@@ -3,8 +3,10 @@
 #include "track_launch.cuh"
 
 namespace gst {
-cudaError_t launch_split_bk(int order, int depth, const TrackArgs& a, size_t tab_bytes, size_t seq_bytes, bool pair,
-                            cudaStream_t st, ChainLaunch* chain) {
-  return launch_split<SPLIT_BK>(order, depth, a, tab_bytes, seq_bytes, pair, st, chain);
+cudaError_t launch_split_bk(int order, int depth, LaunchRequest& rq, cudaStream_t st) {
+  return launch_split<SPLIT_BK>(order, depth, rq, st);
+}
+cudaError_t kernel_info_bk(int order, int depth, bool chain, KernelInfo* out) {
+  return kernel_info_split<SPLIT_BK>(order, depth, chain, out);
 }
 }  // namespace gst

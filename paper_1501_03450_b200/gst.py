@@ -38,8 +38,9 @@ _dp = C.POINTER(C.c_double)
 
 EXPORTS = ["gst_lattice_create", "gst_lattice_destroy", "gst_lattice_steps_per_turn", "gst_bunch_init",
            "gst_bunch_destroy", "gst_track", "gst_polarization", "gst_emittance", "gst_bunch_lost",
-           "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host", "gst_fp64_peak", "gst_selftest_math", "gst_last_error",
-           "gst_set_kernel_variant", "gst_fp64_peak_rrr", "gst_track_pwc", "gst_bunch_last_kernel"]
+           "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host", "gst_last_error",
+           "gst_bunch_set_launch", "gst_bunch_status", "gst_track_pwc", "gst_bunch_last_kernel"]
+LAUNCH_AUTO, LAUNCH_STATIC = 0, 1
 
 
 def lib():
@@ -72,16 +73,11 @@ def lib():
         L.gst_bunch_set_reference.argtypes = [vp, C.POINTER(gst_beam), C.c_int64]
         L.gst_track_host.argtypes = [vp, C.POINTER(_dp), C.c_size_t, C.c_int64, C.c_int, C.c_int, C.c_int, _dp,
                                      C.POINTER(C.c_int64)]
-        L.gst_fp64_peak.argtypes = [_dp, _dp]
-        L.gst_fp64_peak_rrr.argtypes = [_dp, _dp]
-        L.gst_fp64_peak_rrr.restype = C.c_int
-        L.gst_selftest_math.argtypes = [_dp]
-        L.gst_selftest_math.restype = C.c_int
-        L.gst_set_kernel_variant.argtypes = [C.c_int]
-        L.gst_set_kernel_variant.restype = C.c_int
+        L.gst_bunch_set_launch.argtypes = [vp, C.c_int]
+        L.gst_bunch_status.argtypes = [vp, vp]
         for name in ("gst_lattice_create", "gst_bunch_init", "gst_track", "gst_polarization", "gst_emittance",
                      "gst_bunch_lost", "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host",
-                     "gst_fp64_peak"):
+                     "gst_bunch_set_launch", "gst_bunch_status"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -189,6 +185,14 @@ class Bunch:
     def last_kernel(self):
         return lib().gst_bunch_last_kernel(self._h).decode()
 
+    def set_launch(self, mode):
+        """gst_bunch_set_launch: LAUNCH_AUTO (default) or LAUNCH_STATIC (never the rotating launch)."""
+        _check(lib().gst_bunch_set_launch(self._h, int(mode)))
+
+    def status(self, stream=None):
+        """gst_bunch_status: synchronise and raise GstError(ECUDA) if a launch on this bunch failed."""
+        _check(lib().gst_bunch_status(self._h, self._stream(stream)))
+
     def polarization(self, stream=None):
         out = (C.c_double * 4)()
         lost = C.c_int64(0)
@@ -225,34 +229,3 @@ class Bunch:
             self.close()
         except Exception:
             pass
-
-
-KERNEL_FUSED, KERNEL_PAIR, KERNEL_FUSED_STATIC = 0, 1, 2
-
-
-def set_kernel_variant(variant):
-    """gst_set_kernel_variant: KERNEL_FUSED (default) or KERNEL_PAIR (experimental)."""
-    _check(lib().gst_set_kernel_variant(int(variant)))
-
-
-def fp64_peak():
-    """gst_fp64_peak: measured DFMA peak of the current device (TFLOP/s) and the kernel time (ms)."""
-    t = C.c_double(0)
-    ms = C.c_double(0)
-    _check(lib().gst_fp64_peak(C.byref(t), C.byref(ms)))
-    return t.value, ms.value
-
-
-def fp64_peak_rrr():
-    """gst_fp64_peak_rrr: the same with three distinct register operands per DFMA (TFLOP/s, ms)."""
-    t = C.c_double(0)
-    ms = C.c_double(0)
-    _check(lib().gst_fp64_peak_rrr(C.byref(t), C.byref(ms)))
-    return t.value, ms.value
-
-
-def selftest_math():
-    """gst_selftest_math: max residuals of the kernels' rcp / rsqrt in units of 2^-53."""
-    out = (C.c_double * 2)()
-    _check(lib().gst_selftest_math(out))
-    return out[0], out[1]

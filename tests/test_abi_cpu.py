@@ -1,5 +1,6 @@
-"""CPU-side checks of the boundary: the C-ABI library loads and exports every symbol include/gst.h
-declares; the element struct layout matches; compute calls fail loudly without a GPU."""
+"""CPU-side checks of the boundary: the C-ABI library loads and exports every symbol include/gst.h and
+include/gst_diag.h declare, and nothing else; the element struct layout matches; compute calls fail loudly
+without a GPU."""
 import ctypes as C
 import os
 import re
@@ -9,6 +10,7 @@ import pytest
 
 from paper_1501_03450_b200 import build as B
 from paper_1501_03450_b200 import gst
+from paper_1501_03450_b200 import gst_diag
 from paper_1501_03450_b200 import workloads as W
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
@@ -17,11 +19,22 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def test_library_builds_loads_and_exports_every_declared_symbol():
     B.build()
     L = gst.lib()
-    hdr = open(os.path.join(ROOT, "include", "gst.h")).read()
-    declared = set(re.findall(r"\b(gst_[a-z0-9_]+)\s*\(", hdr))
-    assert declared == set(gst.EXPORTS), declared ^ set(gst.EXPORTS)
-    for name in declared:
-        assert hasattr(L, name)
+    declared = {}
+    for header, exports in (("gst.h", gst.EXPORTS), ("gst_diag.h", gst_diag.EXPORTS)):
+        hdr = open(os.path.join(ROOT, "include", header)).read()
+        hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)            # prototypes only, not the prose
+        declared[header] = set(re.findall(r"\b(gst_[a-z0-9_]+)\s*\(", hdr))
+        assert declared[header] == set(exports), declared[header] ^ set(exports)
+        for name in declared[header]:
+            assert hasattr(L, name)
+    # the product header holds the tracking ABI only: diagnostics and test hooks live behind gst_diag.h
+    assert not any(n.startswith("gst_diag_") for n in declared["gst.h"])
+    assert all(n.startswith("gst_diag_") for n in declared["gst_diag.h"])
+    # ... and the library's dynamic symbol table exports exactly the two headers' functions
+    import subprocess
+    out = subprocess.run(["nm", "-D", "--defined-only", gst.LIB_PATH], capture_output=True, text=True).stdout
+    exported = {l.split()[-1] for l in out.splitlines() if " T " in l and l.split()[-1].startswith("gst_")}
+    assert exported == declared["gst.h"] | declared["gst_diag.h"], exported ^ (declared["gst.h"] | declared["gst_diag.h"])
 
 
 def test_struct_layouts_match_the_header():

@@ -35,16 +35,21 @@ def O():
     return oracle
 
 
-def gpu_track(gst, lat, beam, state, n_turns, split, n_slices, depth, chunks=None):
+def gpu_track(gst, lat, beam, state, n_turns, split, n_slices, depth, chunks=None, static=False, want_kernel=None):
     """depth >= 1: gst_track; depth = W.PWC_HALF_SLICE / W.PWC_DKSKD (0 / -1): gst_track_pwc"""
     L = gst.Lattice(lat, beam)
     d = torch.tensor(state, dtype=torch.float64, device="cuda").contiguous()
     b = gst.Bunch(d)
+    if static:
+        b.set_launch(gst.LAUNCH_STATIC)
     for nt in (chunks or [n_turns]):
         if depth >= 1:
             b.track(L, nt, split, n_slices, depth)
         else:
             b.track_pwc(L, nt, split, n_slices, depth)
+    b.status()
+    if want_kernel is not None:
+        assert b.last_kernel() == want_kernel, b.last_kernel()
     pol, nlost = b.polarization()
     emit = b.emittance()
     lost = b.lost()
@@ -174,8 +179,7 @@ def test_pwc_rejects_fourth_order_splits(gst):
     L.close()
 
 
-@pytest.mark.parametrize("variant", ["fused", "pair"])
-def test_thin_fringe_spin_kicks(gst, O, variant):
+def test_thin_fringe_spin_kicks(gst, O):
     """GST_FRINGE (41) P:561 around every thick magnet of the mixed lattice."""
     els = []
     for e in mixed_lattice():
@@ -185,20 +189,15 @@ def test_thin_fringe_spin_kicks(gst, O, variant):
     st = W.gaussian_bunch(17, 200, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
     ref, rlost, _ = O.track(lat, bm, st, 2, W.SPLIT_MATRIX_KICK, 4, 3)
     plain, _, _ = O.track(mixed_lattice(), bm, st, 2, W.SPLIT_MATRIX_KICK, 4, 3)
-    try:
-        gst.set_kernel_variant(gst.KERNEL_PAIR if variant == "pair" else gst.KERNEL_FUSED)
-        got, lost, pol, emit, _ = gpu_track(gst, lat, bm, st, 2, W.SPLIT_MATRIX_KICK, 4, 3)
-    finally:
-        gst.set_kernel_variant(gst.KERNEL_FUSED)
+    got, lost, pol, emit, _ = gpu_track(gst, lat, bm, st, 2, W.SPLIT_MATRIX_KICK, 4, 3)
     assert not rlost.any() and not lost.any()
     assert orbit_err(got, ref) < 2e-12 and spin_err(got, ref) < 2e-12, (orbit_err(got, ref), spin_err(got, ref))
     assert spin_err(plain, ref) > 1e-6                       # the kicks are not a no-op on this bunch
     assert np.array_equal(plain[:6], ref[:6])                # and leave the orbit alone
 
 
-@pytest.mark.parametrize("variant,depth,n_slices", [("fused", 1, 3), ("fused", 4, 8), ("fused", 6, 32), ("pair", 3, 4),
-                                                    ("fused", W.PWC_HALF_SLICE, 4), ("fused", W.PWC_DKSKD, 4)])
-def test_solenoids_in_a_ring(gst, O, variant, depth, n_slices):
+@pytest.mark.parametrize("depth,n_slices", [(1, 3), (3, 4), (4, 8), (6, 32), (W.PWC_HALF_SLICE, 4), (W.PWC_DKSKD, 4)])
+def test_solenoids_in_a_ring(gst, O, depth, n_slices):
     """GST_SOLENOID: body (34), kinetic momentum in Omega (36), fringe kicks (40)."""
     els = list(mixed_lattice())
     els.insert(3, W.solenoid(2.1, 0.2))                      # the paper's 1.3 T x 2.1 m magnet at a few GeV (P:719)
@@ -207,18 +206,13 @@ def test_solenoids_in_a_ring(gst, O, variant, depth, n_slices):
     bm = W.beam(3.0)
     st = W.gaussian_bunch(19, 200, 3.0, 3e-3, 5e-4, 3e-3, 5e-4, 5e-4, 0.05, "sphere")
     ref, rlost, _ = O.track(lat, bm, st, 2, W.SPLIT_BEND_KICK, n_slices, depth)
-    try:
-        gst.set_kernel_variant(gst.KERNEL_PAIR if variant == "pair" else gst.KERNEL_FUSED)
-        got, lost, pol, emit, _ = gpu_track(gst, lat, bm, st, 2, W.SPLIT_BEND_KICK, n_slices, depth)
-    finally:
-        gst.set_kernel_variant(gst.KERNEL_FUSED)
+    got, lost, pol, emit, _ = gpu_track(gst, lat, bm, st, 2, W.SPLIT_BEND_KICK, n_slices, depth)
     assert not rlost.any() and not lost.any()
     assert orbit_err(got, ref) < 2e-12 and spin_err(got, ref) < 2e-12, (orbit_err(got, ref), spin_err(got, ref))
 
 
-@pytest.mark.parametrize("variant,depth,n_slices", [("fused", 1, 3), ("fused", 4, 8), ("fused", 6, 32), ("pair", 3, 4),
-                                                    ("fused", W.PWC_HALF_SLICE, 4), ("fused", W.PWC_DKSKD, 4)])
-def test_rectangular_bends_in_a_ring(gst, O, variant, depth, n_slices):
+@pytest.mark.parametrize("depth,n_slices", [(1, 3), (3, 4), (4, 8), (6, 32), (W.PWC_HALF_SLICE, 4), (W.PWC_DKSKD, 4)])
+def test_rectangular_bends_in_a_ring(gst, O, depth, n_slices):
     """GST_RBEND: rotations (17), fringe map (15) and spin kick (42), body (13), offsets (18)(19)."""
     els = list(mixed_lattice())
     els.insert(2, W.rbend(2.4, 0.12))                         # symmetric
@@ -228,11 +222,7 @@ def test_rectangular_bends_in_a_ring(gst, O, variant, depth, n_slices):
     bm = W.beam(12.0)
     st = W.gaussian_bunch(23, 200, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
     ref, rlost, g_ref = O.track(lat, bm, st, 2, W.SPLIT_BEND_KICK, n_slices, depth)
-    try:
-        gst.set_kernel_variant(gst.KERNEL_PAIR if variant == "pair" else gst.KERNEL_FUSED)
-        got, lost, pol, emit, g_gpu = gpu_track(gst, lat, bm, st, 2, W.SPLIT_BEND_KICK, n_slices, depth)
-    finally:
-        gst.set_kernel_variant(gst.KERNEL_FUSED)
+    got, lost, pol, emit, g_gpu = gpu_track(gst, lat, bm, st, 2, W.SPLIT_BEND_KICK, n_slices, depth)
     assert not rlost.any() and not lost.any()
     assert orbit_err(got, ref) < 2e-12 and spin_err(got, ref) < 2e-12, (orbit_err(got, ref), spin_err(got, ref))
     assert abs(g_gpu - g_ref) < 1e-12 * g_ref                 # the cavity sees the same circumference (arc lengths)
@@ -308,29 +298,6 @@ def test_lost_particles_are_flagged_identically_and_excluded_from_reductions(gst
     assert np.max(np.abs(emit / O.emittance(ref, rlost) - 1)) < 1e-11
 
 
-@pytest.mark.parametrize("split,depth,n_slices", [(W.SPLIT_DRIFT_KICK, 1, 3), (W.SPLIT_BEND_KICK, 4, 8),
-                                                   (W.SPLIT_MATRIX_KICK, 3, 4), (W.SPLIT_BEND_KICK, 6, 32)])
-def test_pair_kernel_variant_is_bit_identical_to_the_fused_kernel(gst, split, depth, n_slices):
-    """GST_KERNEL_PAIR (two threads per particle, csrc/track_pair_kernel.cuh) runs the same arithmetic."""
-    lat = mixed_lattice(ramp=True)
-    bm = W.beam(12.0)
-    for n in (1, 33, 200):                       # one lane, a warp and a lane, several blocks with a ragged tail
-        st = W.gaussian_bunch(11, n, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
-        if n == 200:
-            st[1, 5] = 1.5                       # a lost particle (A15) in a warp that must keep in step
-        fused = gpu_track(gst, lat, bm, st, 3, split, n_slices, depth)
-        try:
-            gst.set_kernel_variant(gst.KERNEL_PAIR)
-            pair = gpu_track(gst, lat, bm, st, 3, split, n_slices, depth)
-        finally:
-            gst.set_kernel_variant(gst.KERNEL_FUSED)
-        assert np.array_equal(fused[1], pair[1])                 # lost flags
-        keep = ~fused[1].astype(bool)
-        assert np.array_equal(fused[0][:, keep], pair[0][:, keep])
-        assert np.array_equal(fused[2], pair[2])                 # polarization over the alive particles
-        assert fused[4] == pair[4]
-
-
 def test_chain_rotation_is_bit_identical_to_the_static_launch(gst):
     """65 553 particles fill the sub-partitions unevenly, so the default launch rotates the warps of particles
     over the warp slots in chunks of turns (csrc/track_chain_kernel.cuh); state, lost flags and the ramping
@@ -341,12 +308,8 @@ def test_chain_rotation_is_bit_identical_to_the_static_launch(gst):
     st = W.gaussian_bunch(29, n, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
     st[1, 5] = 1.5                                   # lost in the first chunk
     st[3, 40000] = -2.0
-    rot = gpu_track(gst, lat, bm, st, 50, W.SPLIT_BEND_KICK, 4, 3)
-    try:
-        gst.set_kernel_variant(gst.KERNEL_FUSED_STATIC)
-        sta = gpu_track(gst, lat, bm, st, 50, W.SPLIT_BEND_KICK, 4, 3)
-    finally:
-        gst.set_kernel_variant(gst.KERNEL_FUSED)
+    rot = gpu_track(gst, lat, bm, st, 50, W.SPLIT_BEND_KICK, 4, 3, want_kernel="track_chain_kernel")
+    sta = gpu_track(gst, lat, bm, st, 50, W.SPLIT_BEND_KICK, 4, 3, static=True, want_kernel="track_kernel")
     assert np.array_equal(rot[1], sta[1]) and rot[1][5] and rot[1][40000]
     keep = ~sta[1].astype(bool)
     assert np.array_equal(rot[0][:, keep], sta[0][:, keep])
@@ -362,13 +325,86 @@ def test_chain_rotation_edge_sizes(gst, n, turns):
     bm = W.beam(12.0)
     st = W.gaussian_bunch(31, n, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
     rot = gpu_track(gst, lat, bm, st, turns, W.SPLIT_MATRIX_KICK, 2, 2)
-    try:
-        gst.set_kernel_variant(gst.KERNEL_FUSED_STATIC)
-        sta = gpu_track(gst, lat, bm, st, turns, W.SPLIT_MATRIX_KICK, 2, 2)
-    finally:
-        gst.set_kernel_variant(gst.KERNEL_FUSED)
+    sta = gpu_track(gst, lat, bm, st, turns, W.SPLIT_MATRIX_KICK, 2, 2, static=True, want_kernel="track_kernel")
     assert not sta[1].any() and np.array_equal(rot[1], sta[1])
     assert np.array_equal(rot[0], sta[0]) and rot[4] == sta[4]
+
+
+@pytest.mark.parametrize("split", [W.SPLIT_DRIFT_KICK, W.SPLIT_BEND_KICK, W.SPLIT_MATRIX_KICK])
+@pytest.mark.parametrize("depth,n_slices", [(1, 1), (2, 2), (4, 8), (6, 32)])
+def test_chain_rotation_every_split_and_low_depths(gst, split, depth, n_slices):
+    """The rotating launch for instantiations whose register count (and hence occupancy) differs from the
+    headline kernel's: the slot numbering must hold for any spread of the blocks over the SMs
+    (csrc/track_chain_kernel.cuh), so state, lost flags and reference energy equal the static launch's."""
+    lat = mixed_lattice(ramp=True)
+    bm = W.beam(12.0)
+    n = 65536 + 17
+    st = W.gaussian_bunch(37, n, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
+    st[1, 77] = 1.5
+    turns = 16 if depth > 4 else 24
+    rot = gpu_track(gst, lat, bm, st, turns, split, n_slices, depth, want_kernel="track_chain_kernel")
+    sta = gpu_track(gst, lat, bm, st, turns, split, n_slices, depth, static=True, want_kernel="track_kernel")
+    assert np.array_equal(rot[1], sta[1]) and rot[1][77]
+    keep = ~sta[1].astype(bool)
+    assert np.array_equal(rot[0][:, keep], sta[0][:, keep])
+    assert np.array_equal(rot[2], sta[2]) and rot[4] == sta[4]
+
+
+def test_failed_rotating_launch_is_reported_by_every_synchronising_call(gst):
+    """Fault injection (include/gst_diag.h): with a poll budget of one, the first warp that has to wait for a
+    hand-off gives up as it would after a hang.  Every call that synchronises must then return GST_ECUDA once,
+    launches enqueued behind the failure must do nothing, and the bunch must be usable again afterwards."""
+    from paper_1501_03450_b200 import gst_diag
+    lat = mixed_lattice(ramp=True)
+    bm = W.beam(12.0)
+    n = 65536
+    st = W.gaussian_bunch(39, n, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
+    want = gpu_track(gst, lat, bm, st, 32, W.SPLIT_BEND_KICK, 4, 3, want_kernel="track_chain_kernel")[0]
+    L = gst.Lattice(lat, bm)
+    calls = {"status": lambda b: b.status(), "polarization": lambda b: b.polarization(),
+             "emittance": lambda b: b.emittance(), "lost": lambda b: b.lost()}
+    for name, call in calls.items():
+        d = torch.tensor(st, dtype=torch.float64, device="cuda").contiguous()
+        b = gst.Bunch(d)
+        gst_diag.chain_poll_limit(b, 1)
+        b.track(L, 32, W.SPLIT_BEND_KICK, 4, 3)
+        assert b.last_kernel() == "track_chain_kernel"
+        b.track(L, 32, W.SPLIT_BEND_KICK, 4, 3)          # enqueued behind the failure: must not run
+        with pytest.raises(gst.GstError) as ei:
+            call(b)
+        assert ei.value.status == gst.ECUDA and "track_chain_kernel" in str(ei.value), (name, str(ei.value))
+        b.status()                                       # reported once, then clear
+        # a checkpoint and a new reference make the bunch whole again (gst.h, "Errors")
+        gst_diag.chain_poll_limit(b, 0)
+        d.copy_(torch.tensor(st, dtype=torch.float64, device="cuda"))
+        b.set_reference(bm, 0)
+        b.track(L, 32, W.SPLIT_BEND_KICK, 4, 3)
+        b.status()
+        assert np.array_equal(d.cpu().numpy(), want), name
+        b.close()
+    L.close()
+
+
+def test_bunch_and_lattice_handles_record_their_device(gst):
+    """Entry points run on the device of their handle whatever the caller's current device is; with one GPU the
+    check is that host memory is refused and that the guard leaves the current device alone."""
+    c = W.config(1)
+    L = gst.Lattice(c["lattice"], c["beam"])
+    with pytest.raises(gst.GstError) as ei:
+        import ctypes
+        host = np.zeros((9, 8))
+        h = ctypes.c_void_p()
+        rows = [ctypes.c_void_p(host[i].ctypes.data) for i in range(9)]
+        gst._check(gst.lib().gst_bunch_init(*rows, 8, ctypes.byref(h)))
+    assert ei.value.status == gst.EINVAL
+    before = torch.cuda.current_device()
+    d = torch.tensor(c["state"], dtype=torch.float64, device="cuda").contiguous()
+    b = gst.Bunch(d)
+    b.track(L, 1, c["split"], 4, 3)
+    b.status()
+    assert torch.cuda.current_device() == before
+    b.close()
+    L.close()
 
 
 def test_fig7_claims_through_the_c_abi(gst, capsys):
@@ -461,15 +497,10 @@ def test_long_lattice_whose_sequence_does_not_fit_shared_memory(gst, O):
     assert len(lat) > 10000
     bm = W.beam(25.0)
     st = W.gaussian_bunch(43, 70, 25.0, 1e-3, 1e-4, 1e-3, 1e-4, 3e-4, 0.05, "sphere")
-    for variant in (gst.KERNEL_FUSED, gst.KERNEL_PAIR):
-        ref, rlost, _ = O.track(lat, bm, st, 1, W.SPLIT_BEND_KICK, 2, 2)
-        try:
-            gst.set_kernel_variant(variant)
-            got, lost, pol, emit, _ = gpu_track(gst, lat, bm, st, 1, W.SPLIT_BEND_KICK, 2, 2)
-        finally:
-            gst.set_kernel_variant(gst.KERNEL_FUSED)
-        assert not rlost.any() and not lost.any()
-        assert orbit_err(got, ref) < 2e-11 and spin_err(got, ref) < 2e-11, (orbit_err(got, ref), spin_err(got, ref))
+    ref, rlost, _ = O.track(lat, bm, st, 1, W.SPLIT_BEND_KICK, 2, 2)
+    got, lost, pol, emit, _ = gpu_track(gst, lat, bm, st, 1, W.SPLIT_BEND_KICK, 2, 2)
+    assert not rlost.any() and not lost.any()
+    assert orbit_err(got, ref) < 2e-11 and spin_err(got, ref) < 2e-11, (orbit_err(got, ref), spin_err(got, ref))
 
 
 def test_two_bunches_on_two_streams(gst):
@@ -618,5 +649,6 @@ def test_config3_full_size_sampled_particles(gst, O):
 
 
 def test_branch_free_rcp_and_rsqrt_are_accurate_to_a_few_ulp(gst):
-    rcp, rsq = gst.selftest_math()
+    from paper_1501_03450_b200 import gst_diag
+    rcp, rsq = gst_diag.selftest_math()
     assert 0 < rcp < 4.0 and 0 < rsq < 4.0, (rcp, rsq)
