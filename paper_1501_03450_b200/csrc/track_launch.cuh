@@ -126,8 +126,16 @@ cudaError_t launch_track(LaunchRequest& rq, cudaStream_t st) {
   return cudaGetLastError();
 }
 
+// -DGST_ONLY_DEPTH=d builds the edge-scheme kernels of Romberg depth d alone (second order; development builds that
+// compile in seconds): every other request fails with cudaErrorNotSupported.
 template <int SPLIT, int ORDER>
 cudaError_t launch_track_depth(int depth, LaunchRequest& rq, cudaStream_t st) {
+#ifdef GST_ONLY_DEPTH
+  if constexpr (ORDER == 2) {
+    if (depth == GST_ONLY_DEPTH) return launch_track<SPLIT, GST_ONLY_DEPTH, 2>(rq, st);
+  }
+  return cudaErrorNotSupported;
+#else
   if (ORDER == 2 && depth == 0) return launch_track<SPLIT, 0, 2>(rq, st);
   if (ORDER == 2 && depth == -1) return launch_track<SPLIT, -1, 2>(rq, st);
   switch (depth) {
@@ -138,6 +146,7 @@ cudaError_t launch_track_depth(int depth, LaunchRequest& rq, cudaStream_t st) {
     case 5: return launch_track<SPLIT, 5, ORDER>(rq, st);
     default: return launch_track<SPLIT, 6, ORDER>(rq, st);
   }
+#endif
 }
 
 template <int SPLIT, int DEPTH, int ORDER>
@@ -155,6 +164,10 @@ cudaError_t kernel_info(bool chain, KernelInfo* out) {
 }
 template <int SPLIT>
 cudaError_t kernel_info_split(int order, int depth, bool chain, KernelInfo* out) {
+#ifdef GST_ONLY_DEPTH
+  if (order == 2 && depth == GST_ONLY_DEPTH) return kernel_info<SPLIT, GST_ONLY_DEPTH, 2>(chain, out);
+  return cudaErrorNotSupported;
+#else
 #define GST_KI(D)                                                          \
   case D: return order == 4 ? kernel_info<SPLIT, D, 4>(chain, out) : kernel_info<SPLIT, D, 2>(chain, out);
   switch (depth) {
@@ -162,6 +175,7 @@ cudaError_t kernel_info_split(int order, int depth, bool chain, KernelInfo* out)
     default: return order == 4 ? kernel_info<SPLIT, 6, 4>(chain, out) : kernel_info<SPLIT, 6, 2>(chain, out);
   }
 #undef GST_KI
+#endif
 }
 
 template <int SPLIT>

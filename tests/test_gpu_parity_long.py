@@ -1,0 +1,211 @@
+"""GPU parity at the BASELINE configurations' own lengths: the CUDA path, through the C ABI, against the CPU oracle
+(long double) on the same seeded inputs.  These are the runs behind north_star's "all 5 configs match the oracle":
+
+  config 2   256 particles x 1000 turns (matrix-kick, cavity, sextupoles); 1e-9 per particle checked at turn 100
+  config 3   the FULL launch bench.py times (65 536 x 1000 turns, rotating kernel); the oracle tracks 256 of its
+             particles, one from every 8th warp of 32 ("chain"), first and last lanes included (particles are
+             independent, so parity on a subset is exact parity for those particles)
+  config 4   256 particles x the full 5000 turns of the ramp (100 keV/turn from G gamma = 45.0 through the intrinsic
+             resonance at 12 + Q_y = 45.43) in chunks of 100 turns, bunch polarization compared AT EVERY REPORT (BASELINE
+             configs[3]: "report the bunch polarization every 100 turns"), gamma_o(n) against its closed form
+  config 5   all 27 (slices, depth) pairs x 3 splits on 64 particles x 10 turns, three of them at the full 100 turns,
+             and the reference run the sweep measures against (fourth-order matrix-kick, 128 slices, depth 6)
+
+Tolerances: north_star's 1e-9 per particle after 100 turns (grown linearly with the turn count beyond that) and 1e-6 on
+the bunch polarization; metrics in tests/parity_metrics.py.  Oracle time on 16 host threads: about three minutes in all.
+With GST_PARITY_REPORT=<file> the measured errors are appended to that file as JSON lines (profiles/rNN_parity_long.md).
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from paper_1501_03450_b200 import workloads as W
+from parity_metrics import orbit_err, orbit_err_per_particle, spin_err
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def gst():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1501_03450_b200 import gst as g
+    g.lib()
+    return g
+
+
+@pytest.fixture(scope="module")
+def O():
+    from oracle import oracle
+    oracle.lib()
+    return oracle
+
+
+def record(name, **values):
+    path = os.environ.get("GST_PARITY_REPORT")
+    if path:
+        with open(path, "a") as f:
+            f.write(json.dumps(dict(test=name, **{k: float(v) for k, v in values.items()})) + "\n")
+
+
+class GpuBunch:
+    """A bunch on the device that can be tracked in pieces and read back between them."""
+
+    def __init__(self, gst, lat, beam, state):
+        self.L = gst.Lattice(lat, beam)
+        self.d = torch.tensor(state, dtype=torch.float64, device="cuda").contiguous()
+        self.b = gst.Bunch(self.d)
+
+    def track(self, turns, split, n_slices, depth):
+        self.b.track(self.L, turns, split, n_slices, depth)
+
+    def read(self):
+        self.b.status()
+        return self.d.cpu().numpy()
+
+    def close(self):
+        self.b.close()
+        self.L.close()
+
+
+def test_config2_thousand_turns(gst, O):
+    c = W.config(2, n_particles=256)
+    args = (c["split"], c["n_slices"], c["depth"])
+    ref100, l100, _ = O.track(c["lattice"], c["beam"], c["state"], 100, *args)
+    ref1000, l1000, _ = O.track(c["lattice"], c["beam"], c["state"], 1000, *args)
+    assert not l100.any() and not l1000.any()
+    g = GpuBunch(gst, c["lattice"], c["beam"], c["state"])
+    g.track(100, *args)
+    got100 = g.read()
+    g.track(900, *args)
+    got1000 = g.read()
+    pol, nlost = g.b.polarization()
+    g.close()
+    assert nlost == 0
+    # north_star: 1e-9 per particle after 100 turns, both metrics
+    assert orbit_err(got100, ref100) < 1e-9 and orbit_err_per_particle(got100, ref100) < 1e-9, \
+        (orbit_err(got100, ref100), orbit_err_per_particle(got100, ref100))
+    assert spin_err(got100, ref100) < 1e-9, spin_err(got100, ref100)
+    # ten times the turns, ten times the tolerance; the bunch polarization to 1e-6
+    assert orbit_err_per_particle(got1000, ref1000) < 1e-8 and spin_err(got1000, ref1000) < 1e-8, \
+        (orbit_err_per_particle(got1000, ref1000), spin_err(got1000, ref1000))
+    rp, _ = O.polarization(ref1000)
+    assert np.max(np.abs(pol - rp)) < 1e-6, (pol, rp)
+    record("config2 256p", orbit_100=orbit_err_per_particle(got100, ref100), spin_100=spin_err(got100, ref100),
+           orbit_1000=orbit_err_per_particle(got1000, ref1000), spin_1000=spin_err(got1000, ref1000),
+           dP_1000=np.max(np.abs(pol - rp)))
+
+
+def test_config3_full_launch_256_sampled_particles(gst, O):
+    c = W.config(3)
+    n = c["state"].shape[1]
+    assert n == 65536 and c["n_turns"] == 1000
+    args = (c["split"], c["n_slices"], c["depth"])
+    g = GpuBunch(gst, c["lattice"], c["beam"], c["state"])
+    g.track(1000, *args)
+    got = g.read()
+    assert g.b.last_kernel() == "track_chain_kernel"          # the kernel bench.py times
+    pol, nlost = g.b.polarization()
+    g.close()
+    assert nlost == 0
+    # one particle from every 8th chain of 32; the lane walks through the warp, first and last lanes included
+    chains = np.arange(0, n // 32, 8)
+    lanes = (np.arange(chains.size) * 7) % 32
+    idx = chains * 32 + lanes
+    idx[0], idx[-1] = 0, n - 1
+    assert idx.size == 256 and (idx % 32 == 0).any() and (idx % 32 == 31).any()
+    ref, rlost, _ = O.track(c["lattice"], c["beam"], c["state"][:, idx], 1000, *args)
+    assert not rlost.any()
+    sub = got[:, idx]
+    assert orbit_err_per_particle(sub, ref) < 1e-8 and spin_err(sub, ref) < 1e-8, \
+        (orbit_err_per_particle(sub, ref), spin_err(sub, ref))
+    rp, _ = O.polarization(ref)
+    assert np.max(np.abs(sub[6:9].mean(axis=1) - rp[:3])) < 1e-6
+    # properties that hold at any size: unit spins; the reduction equals the mean of what was stored
+    assert np.max(np.abs(np.linalg.norm(got[6:9], axis=0) - 1)) < 1e-11
+    assert abs(pol[3] - np.linalg.norm(got[6:9].mean(axis=1))) < 1e-12
+    record("config3 full launch, 256 sampled", orbit_1000=orbit_err_per_particle(sub, ref), spin_1000=spin_err(sub, ref),
+           dP_sample=np.max(np.abs(sub[6:9].mean(axis=1) - rp[:3])), P=pol[3])
+
+
+def test_config4_ramp_with_a_polarization_report_every_100_turns(gst, O):
+    c = W.config(4, n_particles=256)
+    args = (c["split"], c["n_slices"], c["depth"])
+    lat, bm = c["lattice"], c["beam"]
+    cav = lat[lat["type"] == W.RFCAV][0]
+    dEs = np.longdouble(float(cav["volt_eV"])) * np.sin(np.longdouble(float(cav["phi_s"])))
+    E0 = np.longdouble(bm["gamma0"]) * np.longdouble(bm["mass_eV"])
+    g = GpuBunch(gst, lat, bm, c["state"])
+    ref, rlost, g_ref = np.array(c["state"]), None, None
+    worst_dp, worst_g = 0.0, 0.0
+    reports = 50
+    for k in range(1, reports + 1):
+        g.track(100, *args)
+        pol, nlost = g.b.polarization()
+        ref, rlost, g_ref = O.track(lat, bm, ref, 100, *args, lost=rlost, gamma0=g_ref)
+        rp, rl = O.polarization(ref, rlost)
+        assert nlost == 0 and rl == 0
+        worst_dp = max(worst_dp, float(np.max(np.abs(pol - rp))))
+        assert worst_dp < 1e-6, (k, pol, rp)                  # north_star: polarization within 1e-6, at every report
+        g_gpu, turn = g.b.reference()
+        assert turn == 100 * k
+        # A13: E_o(n) = E_o + n dE_s; the kernel's compensated sum keeps gamma_o correctly rounded
+        g_exact = float((E0 + np.longdouble(100 * k) * dEs) / np.longdouble(bm["mass_eV"]))
+        worst_g = max(worst_g, abs(g_gpu - g_exact) / g_exact)
+        assert abs(g_gpu - g_exact) <= 4e-16 * g_exact, (k, g_gpu, g_exact)
+        assert abs(g_gpu - g_ref) <= 3e-15 * g_ref            # the oracle's, rounded to double once per chunk
+    got = g.read()
+    g.close()
+    assert abs(W.G_PROTON * g_gpu - (45.0 + 100 * reports * 1.9108e-4)) < 4e-4      # 45.955: past the resonance at 45.43
+    assert orbit_err_per_particle(got, ref) < 5e-8 and spin_err(got, ref) < 5e-8, \
+        (orbit_err_per_particle(got, ref), spin_err(got, ref))
+    record("config4 256p, 50 reports", orbit_5000=orbit_err_per_particle(got, ref), spin_5000=spin_err(got, ref),
+           worst_dP_any_report=worst_dp, worst_dgamma_rel=worst_g, P_final=pol[3])
+
+
+SPLITS = [W.SPLIT_DRIFT_KICK, W.SPLIT_BEND_KICK, W.SPLIT_MATRIX_KICK]
+
+
+@pytest.mark.parametrize("split", SPLITS)
+def test_config5_every_sweep_point(gst, O, split):
+    c = W.config(5, n_particles=64)
+    pairs = W.sweep_pairs()
+    assert len(pairs) == 27
+    worst = 0.0
+    for n_slices, depth in pairs:
+        ref, rlost, _ = O.track(c["lattice"], c["beam"], c["state"], 10, split, n_slices, depth)
+        g = GpuBunch(gst, c["lattice"], c["beam"], c["state"])
+        g.track(10, split, n_slices, depth)
+        got = g.read()
+        pol, nlost = g.b.polarization()
+        g.close()
+        assert not rlost.any() and nlost == 0
+        eo, es = orbit_err_per_particle(got, ref), spin_err(got, ref)
+        assert eo < 1e-10 and es < 1e-10, (n_slices, depth, eo, es)
+        rp, _ = O.polarization(ref)
+        assert np.max(np.abs(pol - rp)) < 1e-6
+        worst = max(worst, eo, es)
+    record("config5 27 pairs x 10 turns, split %d" % split, worst_orbit_or_spin=worst)
+
+
+@pytest.mark.parametrize("split,n_slices,depth,particles", [
+    (W.SPLIT_DRIFT_KICK, 1, 1, 64), (W.SPLIT_BEND_KICK, 8, 4, 64), (W.SPLIT_MATRIX_KICK, 64, 6, 64),
+    (W.SPLIT_MATRIX_KICK_4, 128, 6, 32)])       # the last one is the reference the committed sweep measures against
+def test_config5_full_hundred_turns(gst, O, split, n_slices, depth, particles):
+    c = W.config(5, n_particles=particles)
+    ref, rlost, _ = O.track(c["lattice"], c["beam"], c["state"], 100, split, n_slices, depth)
+    g = GpuBunch(gst, c["lattice"], c["beam"], c["state"])
+    g.track(100, split, n_slices, depth)
+    got = g.read()
+    pol, nlost = g.b.polarization()
+    g.close()
+    assert not rlost.any() and nlost == 0
+    eo, es = orbit_err_per_particle(got, ref), spin_err(got, ref)
+    assert eo < 1e-9 and es < 1e-9, (eo, es)                  # north_star: 1e-9 after 100 turns
+    rp, _ = O.polarization(ref)
+    assert np.max(np.abs(pol - rp)) < 1e-6
+    record("config5 100 turns split %d N %d d %d" % (split, n_slices, depth), orbit=eo, spin=es, dP=np.max(np.abs(pol - rp)))
