@@ -51,10 +51,17 @@ struct DevTable {
 
 }  // namespace
 
+// One element of the COMPILED lattice: a user element (never a drift except at the end of the ring, never a marker)
+// together with the drift space in front of it.  See compile_lattice().
+struct CompiledElem {
+  gst_element e;
+  double Lpre;     // summed length of the drifts (and skipped markers) between the previous compiled element and this one
+};
+
 struct gst_lattice {
-  std::vector<gst_element> elems;   // as given
-  std::vector<gst_element> uniq;    // de-duplicated
-  std::vector<uint32_t> seq;        // gst::seq_pack(index into uniq, type) per lattice position
+  std::vector<gst_element> elems;   // as given: what gst_lattice_steps_per_turn counts
+  std::vector<CompiledElem> uniq;   // compiled and de-duplicated
+  std::vector<uint32_t> seq;        // gst::seq_pack(index into uniq, type) per position of the compiled sequence
   gst_beam beam;
   int device = 0;                   // the CUDA device the tables live on
   int sms = 0;                      // its SM count
@@ -96,9 +103,11 @@ struct gst_bunch {
 namespace {
 
 // host-side derivation of the per-slice constants of one unique element (a0)
-gst::DevElem derive(const gst_element& e, int n_slices, double C) {
+gst::DevElem derive(const CompiledElem& ce, int n_slices, double C) {
+  const gst_element& e = ce.e;
   gst::DevElem d;
   std::memset(&d, 0, sizeof d);
+  d.Lpre = ce.Lpre;
   d.type = e.type;
   d.N = is_thick(e.type) ? n_slices * e.slice_mult : 1;
   d.L = e.L;
@@ -222,8 +231,8 @@ gst_status validate_track(const gst_lattice* lat, int64_t n_turns, int split, in
   if (split < 0 || split > 5) return fail(GST_EINVAL, "unknown split %d", split);
   if (n_slices < 1 || n_slices > (1 << 20)) return fail(GST_EINVAL, "n_slices must be in 1..2^20");
   if (depth < 1 || depth > 6) return fail(GST_EINVAL, "romberg_depth must be in 1..6");
-  for (const gst_element& e : lat->uniq)
-    if (is_thick(e.type)) {
+  for (const CompiledElem& ce : lat->uniq)
+    if (const gst_element& e = ce.e; is_thick(e.type)) {
       const int64_t N = (int64_t)n_slices * e.slice_mult;          // 2 N must fit an int (half slices of gst_track_pwc)
       if (N > (int64_t)(1 << 30)) return fail(GST_EINVAL, "n_slices*slice_mult = %lld exceeds 2^30", (long long)N);
       if (N % (1LL << (depth - 1)) != 0)
@@ -278,23 +287,54 @@ gst_status gst_lattice_create(const gst_element* elems, size_t n, const gst_beam
   if (!lat) return fail(GST_ENOMEM, "out of host memory");
   lat->elems.assign(elems, elems + n);
   lat->beam = *beam;
-  lat->seq.resize(n);
-  for (size_t i = 0; i < n; ++i) {
-    gst_element e = elems[i];
-    if (!is_thick(e.type)) e.slice_mult = 1;
-    if (e.type == GST_RBEND) lat->C += (e.kn[0] - e.kn[1]) / e.k0;   // design arc length (19)
-    else if (e.type == GST_DRIFT || is_thick(e.type)) lat->C += e.L;
-    else e.L = 0.0;
-    size_t k = 0;
-    for (; k < lat->uniq.size(); ++k)
-      if (std::memcmp(&lat->uniq[k], &e, sizeof e) == 0) break;
-    if (k == lat->uniq.size()) {
-      if (k >= 65535) { delete lat; return fail(GST_EINVAL, "more than 65535 unique elements"); }
-      lat->uniq.push_back(e);
+  // Lattice compilation.  A drift changes no momentum and is exact for any length (29b), so consecutive drifts are one
+  // drift (group property; long straights are cut into many pieces), and a drift followed by a magnet needs the same
+  // sqrt(P^2 - Px^2 - Py^2) as the magnet's own entrance: every run of drifts is folded into the element behind it
+  // (CompiledElem::Lpre -> DevElem::Lpre) and costs that element a handful of multiply-adds instead of an element
+  // dispatch, two reciprocal chains and a square root of its own.  Markers do nothing and are dropped.  The end of the
+  // ring is a hard boundary (the state handed back after a turn is the state at the end of the user's lattice): drifts
+  // that are left there stay one drift element.  The step count of the metric is that of the USER lattice.
+  {
+    double pending = 0.0;
+    auto emit = [&](const gst_element& el, double Lpre) -> bool {
+      CompiledElem ce;
+      std::memset(&ce, 0, sizeof ce);
+      ce.e = el;
+      ce.Lpre = Lpre;
+      size_t k = 0;
+      for (; k < lat->uniq.size(); ++k)
+        if (std::memcmp(&lat->uniq[k], &ce, sizeof ce) == 0) break;
+      if (k == lat->uniq.size()) {
+        if (k >= 65535) return false;
+        lat->uniq.push_back(ce);
+      }
+      lat->seq.push_back(gst::seq_pack((uint32_t)k, el.type));
+      return true;
+    };
+    bool fits = true;
+    for (size_t i = 0; i < n && fits; ++i) {
+      gst_element e = elems[i];
+      if (!is_thick(e.type)) e.slice_mult = 1;
+      if (e.type == GST_RBEND) lat->C += (e.kn[0] - e.kn[1]) / e.k0;   // design arc length (19)
+      else if (e.type == GST_DRIFT || is_thick(e.type)) lat->C += e.L;
+      else e.L = 0.0;
+      if (e.type == GST_RFCAV) lat->cav_dEs.push_back(e.volt_eV * std::sin(e.phi_s));
+      if (e.type == GST_DRIFT) { pending += e.L; continue; }
+      if (e.type == GST_MARKER) continue;
+      fits = emit(e, pending);
+      pending = 0.0;
     }
-    lat->seq[i] = gst::seq_pack((uint32_t)k, e.type);
-    if (e.type == GST_RFCAV) lat->cav_dEs.push_back(e.volt_eV * std::sin(e.phi_s));
+    if (fits && (pending > 0.0 || lat->seq.empty())) {      // what is left at the end of the ring (or a ring of markers)
+      gst_element tail;
+      std::memset(&tail, 0, sizeof tail);
+      tail.type = pending > 0.0 ? GST_DRIFT : GST_MARKER;
+      tail.slice_mult = 1;
+      tail.L = pending;
+      fits = emit(tail, 0.0);
+    }
+    if (!fits) { delete lat; return fail(GST_EINVAL, "more than 65535 unique elements"); }
   }
+  n = lat->seq.size();        // from here on: the compiled sequence
   // the sequence goes up through a pinned staging buffer on a stream of its own, complete when this call returns
   // (a blocking copy from pageable memory may return before its DMA has landed, and streams made with
   // cudaStreamNonBlocking -- torch's -- are not ordered behind the legacy stream)
@@ -469,8 +509,6 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   a.seq = lat->d_seq;
   a.n_unique = (int)lat->uniq.size();
   a.n_seq = (int)lat->seq.size();
-  a.use_smem_seq = 0;
-  a.use_smem_tab = 0;
   a.n = (long long)b->n;
   a.n_turns = n_turns;
   a.E0 = b->E0;
@@ -488,13 +526,8 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   rq.chain.E0 = b->d_chain_E0;
   rq.chain.err = b->d_err;
   rq.poll_limit_override = b->poll_limit_override;
-  cudaError_t ce;
   const int order = (int)split >= 3 ? 4 : 2;
-  switch ((int)split % 3) {
-    case 0: ce = gst::launch_split_dk(order, romberg_depth, rq, st); break;
-    case 1: ce = gst::launch_split_bk(order, romberg_depth, rq, st); break;
-    default: ce = gst::launch_split_mk(order, romberg_depth, rq, st); break;
-  }
+  const cudaError_t ce = gst::launch_tracking((int)split % 3, order, romberg_depth, rq, st);
   if (ce != cudaSuccess) return fail(GST_ECUDA, "track launch: %s", cudaGetErrorString(ce));
   b->last_kernel = rq.kernel;
   // host-side bookkeeping of the reference energy: the same IEEE operations the kernel performs

@@ -140,12 +140,7 @@ gst_status gst_diag_kernel_info(gst_split split, int romberg_depth, int chain, i
   const int order = (int)split >= 3 ? 4 : 2;
   if (chain && order == 4) return fail(GST_EINVAL, "the rotating launch exists for the second-order splits only");
   gst::KernelInfo ki;
-  cudaError_t ce;
-  switch ((int)split % 3) {
-    case 0: ce = gst::kernel_info_dk(order, romberg_depth, chain != 0, &ki); break;
-    case 1: ce = gst::kernel_info_bk(order, romberg_depth, chain != 0, &ki); break;
-    default: ce = gst::kernel_info_mk(order, romberg_depth, chain != 0, &ki); break;
-  }
+  const cudaError_t ce = gst::kernel_info_of((int)split % 3, order, romberg_depth, chain != 0, &ki);
   if (ce != cudaSuccess) return fail(GST_ECUDA, "kernel attributes: %s", cudaGetErrorString(ce));
   if (out_registers) *out_registers = ki.registers;
   if (out_local_bytes) *out_local_bytes = ki.local_bytes;

@@ -127,9 +127,7 @@ __device__ __forceinline__ long long chain_slot_of_block(const ChainArgs& ch, in
 template <int SPLIT, int DEPTH, int ORDER>
 __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_chain_kernel(const TrackArgs a, const ChainArgs ch) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const DevElem* tab;
-  const uint32_t* seq;
-  stage_lattice(a, smem_raw, tab, seq);
+  stage_lattice<false>(a, smem_raw);                     // the planner takes this kernel only when the lattice is resident
   if (*a.err != 0) return;                               // an earlier launch on this bunch failed: leave everything (gst.h)
   const int lane = threadIdx.x & 31;
   const long long slots = (long long)gridDim.x * (TRACK_BLOCK / 32);
@@ -186,7 +184,7 @@ __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_chain_ker
     typename SpinPolicy<DEPTH, SPLIT>::type spin(z);
     const long long t0 = k * ch.chunk_turns;
     const long long t1 = t0 + ch.chunk_turns < a.n_turns ? t0 + ch.chunk_turns : a.n_turns;
-    const bool lost = track_turns<SPLIT, ORDER>(z, ref, pc, spin, t0, t1, tab, seq, a.n_seq, a.G);
+    const bool lost = track_turns<SPLIT, ORDER, false>(z, ref, pc, spin, t0, t1, a, smem_raw);
     if (valid) {
       if (lost) {
         a.lost[j] = 1;

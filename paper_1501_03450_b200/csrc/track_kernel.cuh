@@ -47,6 +47,7 @@ struct __align__(16) DevElem {
   int order;      // highest multipole order present (2..5); 2 if none
   int pure_quad;  // 1 when only kn[0] is non-zero
   double L;       // length
+  double Lpre;    // length of the drift space in front of this element that the lattice compiler merged into it (0: none)
   double ds;      // L / N
   double h, k0;
   // sector bend, exact map over ds
@@ -82,8 +83,6 @@ struct TrackArgs {
   const uint32_t* seq;     // element sequence: (index into tab) << 8 | type, see seq_pack()
   int n_unique;
   int n_seq;
-  int use_smem_seq;
-  int use_smem_tab;         // 0: the table is too big for shared memory and is read from global memory (L1-cached, uniform)
   long long n;
   long long n_turns;
   double E0, E0lo, mass, G;   // reference energy = E0 + E0lo (compensated sum of the cavity gains)
@@ -117,6 +116,10 @@ __device__ __forceinline__ double rsqrt_nr(double x) {
   return fma(y * e, c, y);          // cubic step y (1 + e/2 + 3e^2/8), residual (5/16) e^3 < 2^-58
 }
 
+// domain test of A15 (false for NaN).  Integer compares on the sign-and-exponent word instead of DSETP measured 0.5 %
+// slower, although a DSETP takes two FP64 issue slots.
+__device__ __forceinline__ bool is_pos(double x) { return x > 0.0; }
+
 // reference-particle and per-particle constants that change only when Pt or E0 changes
 struct Ref {
   double E0, mass, p0c, beta0, gamma0, ibeta0, ibg2;  // ibg2 = 1/(beta0 gamma0)^2 = 1/beta0^2 - 1
@@ -130,11 +133,6 @@ struct PCon {
   double tA;    // 2 Pt/(beta0 gamma0)^2 + Pt^2/beta0   (time-of-flight numerator, see drift())
   double tq;    // 1/beta0 - (1/beta0 + Pt)/P, cancellation-free
   double ibpt;  // 1/beta0 + Pt
-  // The last drift's 1/Ps and time-of-flight factor.  A drift changes no momentum, so a drift that directly
-  // follows a drift (long straights are cut into pieces) reuses them instead of two MUFU + Newton chains:
-  // the same numbers, three FMAs.  Cleared by every element that can change Px, Py or Pt.
-  double d_iPs, d_num;
-  bool d_valid;
 };
 
 // A13: E_o <- E_o + dE_s once per turn and cavity.  The spin phase of a turn is 2 pi G gamma_o, so rounding errors of
@@ -171,19 +169,36 @@ __device__ __forceinline__ void pcon_set(PCon& c, double Pt, const Ref& r, doubl
   // (P-1)/beta0 - Pt = [tA - Pt (P-1)]/(P+1),  P-1 = e0/(P+1)
   double ip1 = 1.0 / (c.P + 1.0);
   c.tq = (c.tA - Pt * c.e0 * ip1) * ip1 * c.iP;
-  c.d_valid = false;
 }
 
 // ---------------------------------------------------------------------------------------------
 // quaternions (a10, a11)
 // ---------------------------------------------------------------------------------------------
 // q = (cos(th/2), sin(th/2) w/th) for rotation vector w: both factors are even in th, so they are
-// power series in v = th^2 -- no sqrt, no division, no sincos ("low-order polynomials", here
-// taken to full double precision).  Three tiers by angle; the first is the straight-line path.
+// functions of v = th^2 -- no sqrt, no division, no sincos ("low-order polynomials", here
+// taken to full double precision).  Three tiers by angle; the first is the straight-line path:
+//   tier 1  v <= 1/8 (th <= 0.35 rad per edge: every magnet of the BASELINE rings at >= 8 slices): degree-4
+//           polynomials in v that interpolate cos(sqrt(v)/2) and sin(sqrt(v)/2)/sqrt(v) at the five Chebyshev
+//           nodes of [0, 1/8] (near-minimax; 50-digit fit, coefficients rounded to double, constant terms
+//           1 and 1/2 exactly): error 3.2e-17 absolute on the cosine, 3.2e-18 relative on the sine factor
+//           -- below half an ulp; the degree-6 Taylor pair it replaces costs four more DFMAs per edge
+//   tier 2  v <= 2: Taylor, 10 terms;   tier 3: sincos.
 // The coefficients sit in constant memory so that each DFMA takes its coefficient as a c[bank][offset]
 // operand (a double literal would cost two extra UMOV/MOV instructions per use on sm_100).
-//   QPOLY[2k]   = (-1/4)^k/(2k)!        (cos x,        x^2 = v/4)
-//   QPOLY[2k+1] = (1/2)(-1/4)^k/(2k+1)!  (sin(x)/th)
+//   QPOLY[2k] = coefficient of v^k in the cosine, QPOLY[2k+1] = in sin(x)/th, k = 1..4
+#ifndef GST_QPOLY_DEG
+#define GST_QPOLY_DEG 4
+#endif
+#if GST_QPOLY_DEG == 4
+#define GST_QTIER1 0.125
+static __constant__ double QPOLY[10] = {
+    1.0, 0.5,
+    -0.12499999999999359, -0.02083333333333304,
+    0.0026041666662562613, 0.00026041666664801025,
+    -2.1701379695306356e-05, -1.5500987884264741e-06,
+    9.679713447825894e-08, 5.378467506662951e-09};
+#else   // degree-6 Taylor pair, v <= 1/2: (-1/4)^k/(2k)! and (1/2)(-1/4)^k/(2k+1)!, remainder (v/4)^7/14! < 6e-18
+#define GST_QTIER1 0.5
 static __constant__ double QPOLY[14] = {
     1.0, 0.5,
     -1.0 / 8.0, -0.5 / 24.0,
@@ -192,6 +207,7 @@ static __constant__ double QPOLY[14] = {
     1.0 / (256.0 * 40320.0), 0.5 / (256.0 * 362880.0),
     -1.0 / (1024.0 * 3628800.0), -0.5 / (1024.0 * 39916800.0),
     1.0 / (4096.0 * 479001600.0), 0.5 / (4096.0 * 6227020800.0)};
+#endif
 
 // tiers 2 and 3 (large angle per edge), kept out of line: they are rare and would otherwise be
 // replicated at every call site (instruction-cache footprint)
@@ -221,15 +237,18 @@ static __device__ __noinline__ double2 quat_cs_slow(double v) {
 
 __device__ __forceinline__ Quat quat_from_rotvec(double wx, double wy, double ws) {
   const double v = fma(wx, wx, fma(wy, wy, ws * ws));   // th^2;  x = th/2, x^2 = v/4
-  // tier 1: v <= 0.5 (th <= 0.707), k = 0..6, remainder (v/4)^7/14! < 6e-18
+#if GST_QPOLY_DEG == 4
+  double c = QPOLY[8], s = QPOLY[9];
+#else
   double c = QPOLY[12], s = QPOLY[13];
   c = fma(c, v, QPOLY[10]); s = fma(s, v, QPOLY[11]);
   c = fma(c, v, QPOLY[8]);  s = fma(s, v, QPOLY[9]);
+#endif
   c = fma(c, v, QPOLY[6]);  s = fma(s, v, QPOLY[7]);
   c = fma(c, v, QPOLY[4]);  s = fma(s, v, QPOLY[5]);
   c = fma(c, v, QPOLY[2]);  s = fma(s, v, QPOLY[3]);
   c = fma(c, v, 1.0);       s = fma(s, v, 0.5);
-  if (__builtin_expect(v > 0.5, 0)) {
+  if (__builtin_expect(v > GST_QTIER1, 0)) {     // (a warp vote in front of this branch measured 6 % slower)
     const double2 cs = quat_cs_slow(v);
     c = cs.x; s = cs.y;
   }
@@ -334,26 +353,38 @@ struct State {
   double X, Px, Y, Py, T, Pt, Sx, Sy, Ss;
 };
 
-// a3: exact drift (29b).  T' = 1/beta0 - (1/beta0+Pt)/Ps is evaluated as
-// [(Ps-1)/beta0 - Pt]/Ps with Ps-1 = (Ps^2-1)/(Ps+1) and the O(Pt) terms combined analytically.
-__device__ __forceinline__ bool drift(State& z, double L, PCon& c, const Ref& r) {
-  if (!c.d_valid) {
-    double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
-    double ps2m1 = c.e0 - pt2;
-    double ps2 = 1.0 + ps2m1;
-    double iPs = rsqrt_nr(ps2);
-    double Ps = ps2 * iPs;
-    double iPs1 = rcp_nr(Ps + 1.0);
-    c.d_iPs = iPs;
-    c.d_num = (fma(-pt2, r.ibeta0, c.tA) - z.Pt * ps2m1 * iPs1) * iPs1;
-    c.d_valid = ps2 > 0.0;
-    if (!c.d_valid) return false;
-  }
-  const double LiPs = L * c.d_iPs;
+// Longitudinal momentum at the particle's present transverse momenta: what a drift, the entrance of a bend and the
+// entrance of a drift-kick magnet all start from.  The lattice compiler (gst_api.cu) merges every drift space into
+// the element behind it (DevElem::Lpre), so that this one square root serves the drift AND that element.
+struct Mom {
+  double pt2;     // Px^2 + Py^2
+  double ps2m1;   // Ps^2 - 1, without cancellation
+  double iPs, Ps;
+  bool ok;        // Ps^2 > 0 (A15)
+};
+__device__ __forceinline__ Mom mom_of(const State& z, const PCon& c) {
+  Mom m;
+  m.pt2 = fma(z.Px, z.Px, z.Py * z.Py);
+  m.ps2m1 = c.e0 - m.pt2;
+  const double ps2 = 1.0 + m.ps2m1;
+  m.ok = is_pos(ps2);
+  m.iPs = rsqrt_nr(ps2);
+  m.Ps = ps2 * m.iPs;
+  return m;
+}
+// a3: exact drift (29b) over L.  T' = 1/beta0 - (1/beta0+Pt)/Ps is evaluated as [(Ps-1)/beta0 - Pt]/Ps with
+// Ps-1 = (Ps^2-1)/(Ps+1) and the O(Pt) terms combined analytically; iPs1 = 1/(Ps+1).
+__device__ __forceinline__ void drift_with(State& z, double L, const Mom& m, double iPs1, const PCon& c, const Ref& r) {
+  const double num = (fma(-m.pt2, r.ibeta0, c.tA) - z.Pt * m.ps2m1 * iPs1) * iPs1;
+  const double LiPs = L * m.iPs;
   z.X = fma(LiPs, z.Px, z.X);
   z.Y = fma(LiPs, z.Py, z.Y);
-  z.T = fma(LiPs, c.d_num, z.T);
-  return true;
+  z.T = fma(LiPs, num, z.T);
+}
+__device__ __forceinline__ bool drift(State& z, double L, const PCon& c, const Ref& r) {
+  const Mom m = mom_of(z, c);
+  drift_with(z, L, m, rcp_nr(m.Ps + 1.0), c, r);
+  return m.ok;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -474,15 +505,18 @@ struct BendExact {
   double Pa2, q2, a1k;
   double h, k0, cm, sn, ck, sk, ome;
   bool bad;
-  __device__ __forceinline__ BendExact(State& z, const DevElem& e, const PCon& c)
+  // A = sqrt(Pa^2 - Px^2) is Ps: the drift space merged in front of the magnet (e.Lpre) shares its square root
+  // and its 1/(Ps + 1) with the entrance values A, 1/A and A - 1
+  __device__ __forceinline__ BendExact(State& z, const DevElem& e, const PCon& c, const Ref& r)
       : X(z.X), Px(z.Px), h(e.h), k0(e.k0), cm(e.cm), sn(e.sn), ck(e.ck), sk(e.sk), ome(e.ome) {
-    const double ea = fma(-z.Py, z.Py, c.e0);     // Pa^2 - 1                                  (8)
-    Pa2 = 1.0 + ea;
-    const double a2 = fma(-z.Px, z.Px, Pa2);
-    bad = !(a2 > 0.0);
-    iA = rsqrt_nr(a2);
-    A = a2 * iA;
-    Am1 = fma(-z.Px, z.Px, ea) * rcp_nr(A + 1.0);  // A - 1 without cancellation
+    const Mom m = mom_of(z, c);
+    const double iPs1 = rcp_nr(m.Ps + 1.0);
+    if (e.Lpre != 0.0) drift_with(z, e.Lpre, m, iPs1, c, r);
+    Pa2 = 1.0 + fma(-z.Py, z.Py, c.e0);            // (8)
+    bad = !m.ok;
+    iA = m.iPs;
+    A = m.Ps;
+    Am1 = m.ps2m1 * iPs1;                          // A - 1 without cancellation
     q2 = c.a2p * e.k0 * z.Py;                      // G(gamma-1) (u.b) / P  per unit momentum component
     a1k = fma(c.a1, e.k0, -q2 * z.Py);
   }
@@ -491,7 +525,7 @@ struct BendExact {
     const double dPx = fma(g, sn, -Px * cm);
     const double Pxf = Px + dPx;
     const double f2 = fma(-Pxf, Pxf, Pa2);
-    bad |= !(f2 > 0.0);
+    bad |= !is_pos(f2);
     const double y = rsqrt_nr(f2);
     const double Af = f2 * y;
     const double rr = (Px + Pxf) * rcp_nr(Af + A);
@@ -530,7 +564,7 @@ __device__ __forceinline__ double asin_small(double x) {
 
 template <class Spin>
 __device__ __forceinline__ bool sbend_exact(State& z, const DevElem& e, const PCon& c, const Ref& r, Spin& spin) {
-  BendExact s(z, e, c);
+  BendExact s(z, e, c, r);
   const double A0 = s.A, Am1_0 = s.Am1, Px0 = z.Px;
   spin.run(s, e.N, e.ds);
   // asin(Px0/Pa) - asin(PxN/Pa) = asin(x),  x = (Px0 A_N - Px_N A_0)/Pa^2  (no cancellation)
@@ -551,12 +585,13 @@ template <int ORDER> struct BendTeapot {
   const PCon& c;
   double Ps, iPs, pa2, q2, a1k;
   bool bad;
-  __device__ __forceinline__ BendTeapot(State& z_, const DevElem& e_, const PCon& c_) : z(z_), e(e_), c(c_) {
+  __device__ __forceinline__ BendTeapot(State& z_, const DevElem& e_, const PCon& c_, const Ref& r) : z(z_), e(e_), c(c_) {
+    const Mom m = mom_of(z, c);
+    if (e.Lpre != 0.0) drift_with(z, e.Lpre, m, rcp_nr(m.Ps + 1.0), c, r);
     pa2 = fma(-z.Py, z.Py, 1.0 + c.e0);
-    const double ps2 = fma(-z.Px, z.Px, pa2);
-    bad = !(ps2 > 0.0);
-    iPs = rsqrt_nr(ps2);
-    Ps = ps2 * iPs;
+    bad = !m.ok;
+    iPs = m.iPs;
+    Ps = m.Ps;
     q2 = c.a2p * e.k0 * z.Py;
     a1k = fma(c.a1, e.k0, -q2 * z.Py);
   }
@@ -564,7 +599,7 @@ template <int ORDER> struct BendTeapot {
   __device__ __forceinline__ void curved_drift(const TeapotHalf& t) {
     const double xp = z.Px * iPs;
     const double D = fma(-xp, t.t, 1.0);
-    bad |= !(D > 0.0);
+    bad |= !is_pos(D);
     const double iD = rcp_nr(D);
     // delta q = [(rho+X) tan phi - len Ps D]/(Ps D)
     const double num = t.r_tanmphi + fma(z.X, t.t, t.len * fma(z.Px, t.t, -(Ps - 1.0)));
@@ -575,13 +610,13 @@ template <int ORDER> struct BendTeapot {
     const double Pxn = fma(z.Px, t.c, Ps * t.s);
     Ps = fma(Ps, t.c, -z.Px * t.s);
     z.Px = Pxn;
-    bad |= !(Ps > 0.0);
+    bad |= !is_pos(Ps);
   }
   // kick of (30c) over `len`, then the new longitudinal momentum
   __device__ __forceinline__ void kick(double len) {
     z.Px = fma(-len * e.k0, fma(e.h, z.X, 1.0), z.Px);
     const double ps2 = fma(-z.Px, z.Px, pa2);
-    bad |= !(ps2 > 0.0);
+    bad |= !is_pos(ps2);
     iPs = rsqrt_nr(ps2);
     Ps = ps2 * iPs;
   }
@@ -617,8 +652,8 @@ template <int ORDER> struct BendTeapot {
   }
 };
 template <int ORDER, class Spin>
-__device__ __forceinline__ bool sbend_teapot(State& z, const DevElem& e, const PCon& c, Spin& spin) {
-  BendTeapot<ORDER> s(z, e, c);
+__device__ __forceinline__ bool sbend_teapot(State& z, const DevElem& e, const PCon& c, const Ref& r, Spin& spin) {
+  BendTeapot<ORDER> s(z, e, c, r);
   spin.run(s, e.N, e.ds);
   return !s.bad;
 }
@@ -660,7 +695,7 @@ template <bool PURE, int ORDER> struct MultDK {
   // the cancellation-free form (one more MUFU + 14 FP64 instructions per slice) is kept for whole drifts.
   __device__ __forceinline__ void momenta() {
     const double ps2 = P2 - fma(z.Px, z.Px, z.Py * z.Py);
-    bad |= !(ps2 > 0.0);
+    bad |= !is_pos(ps2);
     iPs = rsqrt_nr(ps2);
     tnum = fma(-c.ibpt, iPs, ibeta0);
   }
@@ -671,8 +706,11 @@ template <bool PURE, int ORDER> struct MultDK {
     a1k = c.a1 * k1;
     ibeta0 = r.ibeta0;
     P2 = 1.0 + c.e0;
-    bad = false;
-    momenta();
+    const Mom m = mom_of(z, c);                    // shared with the drift space merged in front of the magnet
+    if (e.Lpre != 0.0) drift_with(z, e.Lpre, m, rcp_nr(m.Ps + 1.0), c, r);
+    bad = !m.ok;
+    iPs = m.iPs;
+    tnum = fma(-c.ibpt, iPs, ibeta0);
   }
   __device__ __forceinline__ void drift_by(double len) {
     const double l = len * iPs;
@@ -828,7 +866,7 @@ template <bool FOC, int ORDER> struct QuadMK {
   __device__ __forceinline__ void nonlinear(double len) {
     const double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
     const double ps2 = P2 - pt2;
-    bad |= !(ps2 > 0.0);
+    bad |= !is_pos(ps2);
     const double iPs = rsqrt_nr(ps2);
     const double Ps = ps2 * iPs;
     const double t = iPs * rcp_nr(c.P + Ps);         // 1/(Ps (P+Ps))
@@ -858,7 +896,7 @@ template <bool FOC, int ORDER> struct QuadMK {
   template <bool DKSKD> __device__ __forceinline__ void pwc_second() { advance(); }
   __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) {
     const double ps2 = P2 - fma(z.Px, z.Px, z.Py * z.Py);
-    bad |= !(ps2 > 0.0);
+    bad |= !is_pos(ps2);
     const double iPs = rsqrt_nr(ps2);
     const double pb = c.a2p * k1 * (z.Px * z.Y + z.Py * z.X);
     const double wi = -w * iPs;
@@ -891,7 +929,7 @@ struct BendRect {     // body (13): Px falls linearly, X follows sqrt(Pa^2 - Px^
   __device__ __forceinline__ BendRect(State& z_, const DevElem& e, const PCon& c) : z(z_), k0(e.k0), ds(e.ds) {
     Pa2 = fma(-z.Py, z.Py, 1.0 + c.e0);                    // (8)
     const double a2 = fma(-z.Px, z.Px, Pa2);
-    bad = !(a2 > 0.0);
+    bad = !is_pos(a2);
     iA = rsqrt_nr(a2);
     A = a2 * iA;
     q2 = c.a2p * e.k0 * z.Py;
@@ -900,7 +938,7 @@ struct BendRect {     // body (13): Px falls linearly, X follows sqrt(Pa^2 - Px^
   __device__ __forceinline__ void advance() {
     const double Pxf = fma(-ds, k0, z.Px);                 // (13b)
     const double f2 = fma(-Pxf, Pxf, Pa2);
-    bad |= !(f2 > 0.0);
+    bad |= !is_pos(f2);
     const double y = rsqrt_nr(f2);
     const double Af = f2 * y;
     // (13a): rho_b (A_f - A) = rho_b (Px - Px_f)(Px + Px_f)/(A_f + A) = ds (Px + Px_f)/(A_f + A)
@@ -929,7 +967,7 @@ __device__ __forceinline__ bool rbend_rotate(State& z, const DevElem& e, int k, 
   z.T = fma(-c.ibpt * iPs, q, z.T);                        // (17e), sign of reading A5
   z.X = z.X * e.rb_sec[k] * rcp_nr(den);                   // (17a)
   z.Px = fma(z.Px, e.rb_c[k], Ps * e.rb_s[k]);             // (17b)
-  return ps2 > 0.0 && den > 0.0;
+  return is_pos(ps2) && is_pos(den);
 }
 // thin-fringe orbit map (15), b = +-k0
 __device__ __forceinline__ bool rbend_fringe(State& z, double b, const PCon& c) {
@@ -944,7 +982,7 @@ __device__ __forceinline__ bool rbend_fringe(State& z, double b, const PCon& c) 
   z.Py = fma(-b * xp * id, Yf, z.Py);                                                               // (15d)
   z.T = fma(-0.5 * b * c.ibpt * xp * iPs * iPs * fma(-yp, yp, 1.0) * id * id, Y2, z.T);             // (15e)
   z.Y = Yf;
-  return ps2 > 0.0 && arg > 0.0;
+  return is_pos(ps2) && is_pos(arg);
 }
 template <class Spin>
 __device__ __forceinline__ bool rbend(State& z, const DevElem& e, const PCon& c, const Ref& r, double G, Spin& spin) {
@@ -991,7 +1029,7 @@ struct Solenoid {
     two_eta = e.k0;
     const double kx = fma(eta, z.Y, z.Px), ky = fma(-eta, z.X, z.Py);
     const double ps2 = 1.0 + c.e0 - fma(kx, kx, ky * ky);
-    bad = !(ps2 > 0.0);
+    bad = !is_pos(ps2);
     iPs = rsqrt_nr(bad ? 1.0 : ps2);
     Ps = ps2 * iPs;
     sincos(eta * iPs * e.ds, &sn, &cs);
@@ -1018,7 +1056,7 @@ struct Solenoid {
   __device__ __forceinline__ void fringe(double sign, double& wx, double& wy, double& ws) {
     const double kx = fma(0.5 * eta, z.Y, z.Px), ky = fma(-0.5 * eta, z.X, z.Py);
     const double ps2 = 1.0 + c.e0 - fma(kx, kx, ky * ky);
-    bad |= !(ps2 > 0.0);
+    bad |= !is_pos(ps2);
     const double ips = rsqrt_nr(ps2);
     const double proj = c.a2p * fma(z.X, kx, z.Y * ky);       // G(gamma-1)(X kx + Y ky)/P^2
     const double pre = sign * eta * ips;
@@ -1048,33 +1086,23 @@ __device__ __forceinline__ bool solenoid(State& z, const DevElem& e, const PCon&
 
 static __constant__ double FRINGE_INV_M[4] = {1.0 / 2.0, 1.0 / 3.0, 1.0 / 4.0, 1.0 / 5.0};
 
-// The tests are ordered by how often each type occurs in a ring (drifts, quadrupoles, bends, thin lenses).
+// the element types that take a merged drift space in front of them the plain way (see element_step)
 template <int SPLIT, int ORDER, class Spin>
-__device__ __forceinline__ bool element_step(int type, State& z, const DevElem& e, PCon& pc, Ref& ref, double G, Spin& spin) {
-  if (type == K_DRIFT) return drift(z, e.L, pc, ref);
-  if (type != K_MARKER && type != K_SNAKE) pc.d_valid = false;     // the momenta may change: the cached drift factors expire
-  if (type == K_QUAD) {
-    if (SPLIT == SPLIT_MK) return quad_mk<ORDER>(z, e, pc, spin);
-    return mult_dk<ORDER>(z, e, pc, ref, spin);
-  }
-  if (type == K_SBEND) {
-    if (SPLIT == SPLIT_DK) return sbend_teapot<ORDER>(z, e, pc, spin);
-    return sbend_exact(z, e, pc, ref, spin);
-  }
+__device__ __forceinline__ bool element_step_other(int type, State& z, const DevElem& e, PCon& pc, Ref& ref, double G, Spin& spin) {
+  if (type == K_QUAD) return quad_mk<ORDER>(z, e, pc, spin);
   if (type == K_THIN) {   // A10: half kick, spin, half kick
     double bx, by, wx, wy, ws;
     mult_field(e, z.X, z.Y, bx, by);
     z.Px = fma(-0.5, by, z.Px);
     z.Py = fma(0.5, bx, z.Py);
     const double ps2 = 1.0 + pc.e0 - fma(z.Px, z.Px, z.Py * z.Py);
-    const bool ok = ps2 > 0.0;
+    const bool ok = is_pos(ps2);
     omega_straight(1.0, z.Px, z.Py, rsqrt_nr(ok ? ps2 : 1.0), bx, by, pc, wx, wy, ws);
     spin.thin(wx, wy, ws);
     z.Px = fma(-0.5, by, z.Px);
     z.Py = fma(0.5, bx, z.Py);
     return ok;
   }
-  if (type == K_MULT) return mult_dk<ORDER>(z, e, pc, ref, spin);
   if (type == K_RF) {     // A12, A13
     double krf = e.krf_over_beta * ref.beta0;
     double dE = e.volt * sin(fma(e.sign * krf, z.T, e.phi_s));
@@ -1109,6 +1137,23 @@ __device__ __forceinline__ bool element_step(int type, State& z, const DevElem& 
   return true;
 }
 
+// One element of the COMPILED sequence (gst_api.cu: compile_lattice): drift spaces never come alone -- consecutive
+// ones are merged and each run is handed to the element behind it as e.Lpre -- except at the end of the ring, and
+// markers are gone.  Bends and drift-kick magnets take their Lpre themselves, sharing its square root with their own
+// entrance values; every other type drifts first.  The tests are ordered by how often each type occurs in a ring.
+template <int SPLIT, int ORDER, class Spin>
+__device__ __forceinline__ bool element_step(int type, State& z, const DevElem& e, PCon& pc, Ref& ref, double G, Spin& spin) {
+  if (type == K_QUAD && SPLIT != SPLIT_MK) return mult_dk<ORDER>(z, e, pc, ref, spin);
+  if (type == K_SBEND) {
+    if (SPLIT == SPLIT_DK) return sbend_teapot<ORDER>(z, e, pc, ref, spin);
+    return sbend_exact(z, e, pc, ref, spin);
+  }
+  if (type == K_DRIFT) return drift(z, e.L, pc, ref);
+  if (type == K_MULT) return mult_dk<ORDER>(z, e, pc, ref, spin);
+  bool ok = true;
+  if (e.Lpre != 0.0) ok = drift(z, e.Lpre, pc, ref);
+  return element_step_other<SPLIT, ORDER>(type, z, e, pc, ref, G, spin) && ok;
+}
 // ---------------------------------------------------------------------------------------------
 // the kernel
 // ---------------------------------------------------------------------------------------------
@@ -1124,72 +1169,111 @@ constexpr int TRACK_MIN_BLOCKS = 8;
 // faster; every other instantiation is equal or slightly slower that way (profiles/r01_notes.md).
 __host__ __device__ constexpr int track_min_blocks(int split, int order) { return (split == SPLIT_MK && order == 4) ? 6 : TRACK_MIN_BLOCKS; }
 
-// a0: stage the unique-element table and the sequence into shared memory, each when it fits (host plan: track_launch.cuh)
-__device__ __forceinline__ void stage_lattice(const TrackArgs& a, unsigned char* smem_raw, const DevElem*& tab,
-                                              const uint32_t*& seq) {
-  tab = a.tab;
-  seq = a.seq;
-  size_t off = 0;
-  if (a.use_smem_tab) {
+// a0: the lattice is ALWAYS read from shared memory (LDS; element records and sequence entries through a pointer that
+// may point to global or shared memory measured 3 % slower).  Two layouts of the dynamic shared memory, chosen on the
+// host (track_launch.cuh: plan_smem) and compiled as two kernels:
+//   RESIDENT   [unique-element table][sequence], staged once per block -- every BASELINE ring (12-20 records, <= 2.3 kB
+//              of sequence); needs both to fit the block's budget
+//   STREAMED   per warp [one DevElem][window of SEQ_WINDOW sequence entries]: the warp copies each element's record
+//              from global memory before the element (3 coalesced loads per lane) and refills its window every
+//              SEQ_WINDOW elements -- rings with hundreds of individually powered magnets or tens of thousands of elements
+constexpr int SEQ_WINDOW = 64;
+constexpr size_t STREAM_BYTES_PER_WARP = sizeof(DevElem) + SEQ_WINDOW * sizeof(uint32_t);
+
+template <bool STREAMED>
+__device__ __forceinline__ void stage_lattice(const TrackArgs& a, unsigned char* smem_raw) {
+  if (!STREAMED) {
     const int nw = a.n_unique * (int)(sizeof(DevElem) / sizeof(double));
     const double* src = reinterpret_cast<const double*>(a.tab);
     double* dst = reinterpret_cast<double*>(smem_raw);
     for (int i = threadIdx.x; i < nw; i += blockDim.x) dst[i] = src[i];
-    tab = reinterpret_cast<const DevElem*>(smem_raw);
-    off = (size_t)a.n_unique * sizeof(DevElem);
-  }
-  if (a.use_smem_seq) {
-    uint32_t* sseq = reinterpret_cast<uint32_t*>(smem_raw + off);
+    uint32_t* sseq = reinterpret_cast<uint32_t*>(smem_raw + (size_t)a.n_unique * sizeof(DevElem));
     for (int i = threadIdx.x; i < a.n_seq; i += blockDim.x) sseq[i] = a.seq[i];
-    seq = sseq;
   }
   __syncthreads();
 }
 
-// Turns [t0, t1) of the ring for one particle.  The turn and element loops run to the end for every thread, so
-// that their counters, the sequence loads and the type dispatch are warp-uniform (uniform registers, no divergence
-// bookkeeping); a particle that is lost (A15) goes on with the reference orbit and nothing of it is stored (R6).
-template <int SPLIT, int ORDER, class Spin>
+// Turns [t0, t1) of the ring for one particle.  The turn and element loops run to the end for every thread of the
+// warp (also for lanes without a particle, which carry a particle on the reference orbit), so that their counters, the
+// sequence loads and the type dispatch are warp-uniform (uniform registers, no divergence bookkeeping) and the warp can
+// copy element records together; a particle that is lost (A15) goes on with the reference orbit and nothing of it is
+// stored (R6).
+template <int SPLIT, int ORDER, bool STREAMED, class Spin>
 __device__ __forceinline__ bool track_turns(State& z, Ref& ref, PCon& pc, Spin& spin, long long t0, long long t1,
-                                            const DevElem* tab, const uint32_t* seq, int n_seq, double G) {
+                                            const TrackArgs& a, unsigned char* smem_raw) {
   bool lost = false;
-  uint32_t nxt = seq[0];
-  for (long long turn = t0; turn < t1; ++turn) {
+  const int n_seq = a.n_seq;
+  if (!STREAMED) {
+    const DevElem* tab = reinterpret_cast<const DevElem*>(smem_raw);
+    const uint32_t* seq = reinterpret_cast<const uint32_t*>(smem_raw + (size_t)a.n_unique * sizeof(DevElem));
+    uint32_t nxt = seq[0];
+    for (long long turn = t0; turn < t1; ++turn) {
 #pragma unroll 1
-    for (int ie = 0; ie < n_seq; ++ie) {
-      const uint32_t cur = nxt;
-      nxt = seq[ie + 1 < n_seq ? ie + 1 : 0];          // next element's entry, one element ahead
-      const DevElem& e = tab[cur >> 8];
-      const bool ok = element_step<SPLIT, ORDER>((int)(cur & 0xffu), z, e, pc, ref, G, spin);
-      if (!ok) {
-        lost = true;
-        z.X = z.Px = z.Y = z.Py = z.T = z.Pt = 0.0;
-        pcon_set(pc, 0.0, ref, G);
+      for (int ie = 0; ie < n_seq; ++ie) {
+        const uint32_t cur = nxt;
+        nxt = seq[ie + 1 < n_seq ? ie + 1 : 0];          // next element's entry, one element ahead
+        const bool ok = element_step<SPLIT, ORDER>((int)(cur & 0xffu), z, tab[cur >> 8], pc, ref, a.G, spin);
+        if (!ok) {
+          lost = true;
+          z.X = z.Px = z.Y = z.Py = z.T = z.Pt = 0.0;
+          pcon_set(pc, 0.0, ref, a.G);
+        }
+      }
+    }
+  } else {
+    const int lane = threadIdx.x & 31;
+    unsigned char* mine = smem_raw + (threadIdx.x >> 5) * STREAM_BYTES_PER_WARP;
+    double* rec = reinterpret_cast<double*>(mine);
+    uint32_t* win = reinterpret_cast<uint32_t*>(mine + sizeof(DevElem));
+    for (long long turn = t0; turn < t1; ++turn) {
+#pragma unroll 1
+      for (int ie = 0; ie < n_seq; ++ie) {
+        if ((ie & (SEQ_WINDOW - 1)) == 0) {               // refill the window of sequence entries
+          __syncwarp();
+          for (int k = lane; k < SEQ_WINDOW && ie + k < n_seq; k += 32) win[k] = a.seq[ie + k];
+          __syncwarp();
+        }
+        const uint32_t cur = win[ie & (SEQ_WINDOW - 1)];
+        const double* src = reinterpret_cast<const double*>(a.tab + (cur >> 8));
+        __syncwarp();                                     // everybody is done with the previous record
+        for (int k = lane; k < (int)(sizeof(DevElem) / sizeof(double)); k += 32) rec[k] = src[k];
+        __syncwarp();
+        const bool ok = element_step<SPLIT, ORDER>((int)(cur & 0xffu), z, *reinterpret_cast<const DevElem*>(mine), pc, ref,
+                                                   a.G, spin);
+        if (!ok) {
+          lost = true;
+          z.X = z.Px = z.Y = z.Py = z.T = z.Pt = 0.0;
+          pcon_set(pc, 0.0, ref, a.G);
+        }
       }
     }
   }
   return lost;
 }
 
-template <int SPLIT, int DEPTH, int ORDER>
+template <int SPLIT, int DEPTH, int ORDER, bool STREAMED>
 __global__ void __launch_bounds__(TRACK_BLOCK, track_min_blocks(SPLIT, ORDER)) track_kernel(const TrackArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const DevElem* tab;
-  const uint32_t* seq;
-  stage_lattice(a, smem_raw, tab, seq);
+  stage_lattice<STREAMED>(a, smem_raw);
+  if (*a.err != 0) return;                               // an earlier launch on this bunch failed: leave everything (gst.h)
   const long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= a.n) return;
-  if (*a.err != 0 || a.lost[j]) return;
+  const bool valid = j < a.n && !a.lost[j];
+  if (!__any_sync(0xffffffffu, valid)) return;           // a warp without particles (the other lanes keep in step)
   State z;
-  z.X = a.p[0][j]; z.Px = a.p[1][j]; z.Y = a.p[2][j]; z.Py = a.p[3][j]; z.T = a.p[4][j]; z.Pt = a.p[5][j];
-  z.Sx = a.p[6][j]; z.Sy = a.p[7][j]; z.Ss = a.p[8][j];
+  z.X = z.Px = z.Y = z.Py = z.T = z.Pt = 0.0;
+  z.Sx = 0.0; z.Sy = 1.0; z.Ss = 0.0;
+  if (valid) {
+    z.X = a.p[0][j]; z.Px = a.p[1][j]; z.Y = a.p[2][j]; z.Py = a.p[3][j]; z.T = a.p[4][j]; z.Pt = a.p[5][j];
+    z.Sx = a.p[6][j]; z.Sy = a.p[7][j]; z.Ss = a.p[8][j];
+  }
   Ref ref;
   ref_set(ref, a.E0, a.mass);
   ref.E0lo = a.E0lo;
   PCon pc;
   pcon_set(pc, z.Pt, ref, a.G);
   typename SpinPolicy<DEPTH, SPLIT>::type spin(z);
-  const bool lost = track_turns<SPLIT, ORDER>(z, ref, pc, spin, 0, a.n_turns, tab, seq, a.n_seq, a.G);
+  const bool lost = track_turns<SPLIT, ORDER, STREAMED>(z, ref, pc, spin, 0, a.n_turns, a, smem_raw);
+  if (!valid) return;
   if (lost) { a.lost[j] = 1; return; }
   a.p[0][j] = z.X; a.p[1][j] = z.Px; a.p[2][j] = z.Y; a.p[3][j] = z.Py; a.p[4][j] = z.T; a.p[5][j] = z.Pt;
   a.p[6][j] = z.Sx; a.p[7][j] = z.Sy; a.p[8][j] = z.Ss;

@@ -23,29 +23,54 @@ struct LaunchRequest {
   const char* kernel = "";      // out: name of the kernel launched
 };
 
-// order = 2 or 4 (composition of the slice maps); depth >= 1: Romberg depth, 0 / -1: mid-slice PWC orderings
-cudaError_t launch_split_dk(int order, int depth, LaunchRequest& rq, cudaStream_t st);
-cudaError_t launch_split_bk(int order, int depth, LaunchRequest& rq, cudaStream_t st);
-cudaError_t launch_split_mk(int order, int depth, LaunchRequest& rq, cudaStream_t st);
-
 // resources of one instantiation (gst_diag_kernel_info): what bench.py checks its flop model's capture against
 struct KernelInfo { int registers = 0, local_bytes = 0, blocks_per_sm = 0; };
-cudaError_t kernel_info_dk(int order, int depth, bool chain, KernelInfo* out);
-cudaError_t kernel_info_bk(int order, int depth, bool chain, KernelInfo* out);
-cudaError_t kernel_info_mk(int order, int depth, bool chain, KernelInfo* out);
+
+// The template instantiations (3 splits x 2 orders x 6 depths + 2 mid-slice orderings, each as a resident and a
+// streamed kernel, plus the rotating kernels) are compiled in nine translation units that build in parallel:
+// track_inst.cu with -DGST_TU_SPLIT=s -DGST_TU_GROUP=g, where group 0 = second order, depths 1-3 and the two mid-slice
+// orderings, 1 = second order, depths 4-6, 2 = fourth order.  order = 2 or 4 (composition of the slice maps);
+// depth >= 1: Romberg depth, 0 / -1: mid-slice PWC orderings.
+#define GST_DECLARE_TU(S, G)                                                                        \
+  cudaError_t launch_tu_##S##_##G(int order, int depth, LaunchRequest& rq, cudaStream_t st);         \
+  cudaError_t kernel_info_tu_##S##_##G(int order, int depth, bool chain, KernelInfo* out);
+GST_DECLARE_TU(0, 0) GST_DECLARE_TU(0, 1) GST_DECLARE_TU(0, 2)
+GST_DECLARE_TU(1, 0) GST_DECLARE_TU(1, 1) GST_DECLARE_TU(1, 2)
+GST_DECLARE_TU(2, 0) GST_DECLARE_TU(2, 1) GST_DECLARE_TU(2, 2)
+#undef GST_DECLARE_TU
+
+inline int tu_group(int order, int depth) { return order == 4 ? 2 : (depth >= 4 ? 1 : 0); }
+#define GST_DISPATCH_TU(FN, ...)                                                  \
+  switch (split3 * 3 + tu_group(order, depth)) {                                  \
+    case 0: return FN##_0_0(__VA_ARGS__);                                         \
+    case 1: return FN##_0_1(__VA_ARGS__);                                         \
+    case 2: return FN##_0_2(__VA_ARGS__);                                         \
+    case 3: return FN##_1_0(__VA_ARGS__);                                         \
+    case 4: return FN##_1_1(__VA_ARGS__);                                         \
+    case 5: return FN##_1_2(__VA_ARGS__);                                         \
+    case 6: return FN##_2_0(__VA_ARGS__);                                         \
+    case 7: return FN##_2_1(__VA_ARGS__);                                         \
+    default: return FN##_2_2(__VA_ARGS__);                                        \
+  }
+// split3 = SPLIT_DK / SPLIT_BK / SPLIT_MK
+inline cudaError_t launch_tracking(int split3, int order, int depth, LaunchRequest& rq, cudaStream_t st) {
+  GST_DISPATCH_TU(launch_tu, order, depth, rq, st)
+}
+inline cudaError_t kernel_info_of(int split3, int order, int depth, bool chain, KernelInfo* out) {
+  GST_DISPATCH_TU(kernel_info_tu, order, depth, chain, out)
+}
+#undef GST_DISPATCH_TU
 
 #ifdef GST_LAUNCH_IMPL
 namespace {
 
-// shared memory of one block: table [sequence when it fits]
-struct SmemPlan { size_t bytes; int use_smem_tab, use_smem_seq; };
+// shared memory of one block (track_kernel.cuh: stage_lattice): table and sequence resident when both fit the budget
+// (24 kB per block keeps 8 blocks per SM), else one record and one sequence window per warp
+struct SmemPlan { size_t bytes; bool streamed; };
 inline SmemPlan plan_smem(size_t tab_bytes, size_t seq_bytes, size_t budget) {
   SmemPlan p;
-  // the table first (read at every element), then the sequence; what does not fit stays in global memory
-  p.use_smem_tab = (tab_bytes <= budget) ? 1 : 0;
-  const size_t with_tab = p.use_smem_tab ? tab_bytes : 0;
-  p.use_smem_seq = (with_tab + seq_bytes <= budget) ? 1 : 0;
-  p.bytes = with_tab + (p.use_smem_seq ? seq_bytes : 0);
+  p.streamed = tab_bytes + seq_bytes > budget;
+  p.bytes = p.streamed ? (size_t)(TRACK_BLOCK / 32) * STREAM_BYTES_PER_WARP : tab_bytes + seq_bytes;
   return p;
 }
 
@@ -85,13 +110,10 @@ template <int SPLIT, int DEPTH, int ORDER>
 cudaError_t launch_track(LaunchRequest& rq, cudaStream_t st) {
   TrackArgs& a = rq.args;
   const SmemPlan p = plan_smem(rq.tab_bytes, rq.seq_bytes, 24 * 1024);
-  a.use_smem_seq = p.use_smem_seq;
-  a.use_smem_tab = p.use_smem_tab;
   if constexpr (ORDER == 2 && DEPTH >= 1) {
-    if (rq.allow_chain) {   // T1c: the same arithmetic with the chains rotating over all resident warp slots
+    if (rq.allow_chain && !p.streamed) {   // T1c: the same arithmetic with the chains rotating over all resident warp slots
       auto ck = track_chain_kernel<SPLIT, DEPTH, ORDER>;
       int per_sm = 0;
-      if (p.bytes > 48 * 1024) cudaFuncSetAttribute(ck, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
       cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ck, TRACK_BLOCK, p.bytes);
       if (e != cudaSuccess) return e;
       // the grid never exceeds what is co-resident; when the occupancy is higher than the launch bound asks for, the
@@ -115,43 +137,16 @@ cudaError_t launch_track(LaunchRequest& rq, cudaStream_t st) {
     }
   }
   // T1: one thread per particle; shared memory kept small so that 8 blocks of 64 threads stay resident
-  auto kern = track_kernel<SPLIT, DEPTH, ORDER>;
-  if (p.bytes > 48 * 1024) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p.bytes);
-    if (e != cudaSuccess) return e;
-  }
+  auto kern = p.streamed ? track_kernel<SPLIT, DEPTH, ORDER, true> : track_kernel<SPLIT, DEPTH, ORDER, false>;
   const unsigned blocks = (unsigned)((a.n + TRACK_BLOCK - 1) / TRACK_BLOCK);
   kern<<<blocks, TRACK_BLOCK, p.bytes, st>>>(a);
   rq.kernel = "track_kernel";
   return cudaGetLastError();
 }
 
-// -DGST_ONLY_DEPTH=d builds the edge-scheme kernels of Romberg depth d alone (second order; development builds that
-// compile in seconds): every other request fails with cudaErrorNotSupported.
-template <int SPLIT, int ORDER>
-cudaError_t launch_track_depth(int depth, LaunchRequest& rq, cudaStream_t st) {
-#ifdef GST_ONLY_DEPTH
-  if constexpr (ORDER == 2) {
-    if (depth == GST_ONLY_DEPTH) return launch_track<SPLIT, GST_ONLY_DEPTH, 2>(rq, st);
-  }
-  return cudaErrorNotSupported;
-#else
-  if (ORDER == 2 && depth == 0) return launch_track<SPLIT, 0, 2>(rq, st);
-  if (ORDER == 2 && depth == -1) return launch_track<SPLIT, -1, 2>(rq, st);
-  switch (depth) {
-    case 1: return launch_track<SPLIT, 1, ORDER>(rq, st);
-    case 2: return launch_track<SPLIT, 2, ORDER>(rq, st);
-    case 3: return launch_track<SPLIT, 3, ORDER>(rq, st);
-    case 4: return launch_track<SPLIT, 4, ORDER>(rq, st);
-    case 5: return launch_track<SPLIT, 5, ORDER>(rq, st);
-    default: return launch_track<SPLIT, 6, ORDER>(rq, st);
-  }
-#endif
-}
-
 template <int SPLIT, int DEPTH, int ORDER>
 cudaError_t kernel_info(bool chain, KernelInfo* out) {
-  const void* f = (const void*)track_kernel<SPLIT, DEPTH, ORDER>;
+  const void* f = (const void*)track_kernel<SPLIT, DEPTH, ORDER, false>;
   if constexpr (ORDER == 2 && DEPTH >= 1) {
     if (chain) f = (const void*)track_chain_kernel<SPLIT, DEPTH, ORDER>;
   }
@@ -162,28 +157,6 @@ cudaError_t kernel_info(bool chain, KernelInfo* out) {
   out->local_bytes = (int)at.localSizeBytes;
   return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&out->blocks_per_sm, f, TRACK_BLOCK, 0);
 }
-template <int SPLIT>
-cudaError_t kernel_info_split(int order, int depth, bool chain, KernelInfo* out) {
-#ifdef GST_ONLY_DEPTH
-  if (order == 2 && depth == GST_ONLY_DEPTH) return kernel_info<SPLIT, GST_ONLY_DEPTH, 2>(chain, out);
-  return cudaErrorNotSupported;
-#else
-#define GST_KI(D)                                                          \
-  case D: return order == 4 ? kernel_info<SPLIT, D, 4>(chain, out) : kernel_info<SPLIT, D, 2>(chain, out);
-  switch (depth) {
-    GST_KI(1) GST_KI(2) GST_KI(3) GST_KI(4) GST_KI(5)
-    default: return order == 4 ? kernel_info<SPLIT, 6, 4>(chain, out) : kernel_info<SPLIT, 6, 2>(chain, out);
-  }
-#undef GST_KI
-#endif
-}
-
-template <int SPLIT>
-cudaError_t launch_split(int order, int depth, LaunchRequest& rq, cudaStream_t st) {
-  if (order == 4) return launch_track_depth<SPLIT, 4>(depth, rq, st);
-  return launch_track_depth<SPLIT, 2>(depth, rq, st);
-}
-
 }  // namespace
 #endif  // GST_LAUNCH_IMPL
 
