@@ -59,3 +59,110 @@ def test_shard_bounds_cover_everything_once():
             b = [D.shard_bounds(n, r, w) for r in range(w)]
             assert b[0][0] == 0 and b[-1][1] == n
             assert all(b[i][1] == b[i + 1][0] for i in range(w - 1))
+
+
+# ---------------------------------------------------------------------------------------------
+# bench.py's own N>1 code path (rank-local bunches, barriers, max-over-ranks timing, the 5-double all-reduce) on two
+# gloo ranks.  The tracking call is injected HERE: a stand-in for bench.CudaMachine that "tracks" by sleeping.
+# ---------------------------------------------------------------------------------------------
+class _StubSampler:
+    def start(self):
+        pass
+
+    def stop(self):
+        return {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+
+
+class _StubMachine:
+    dist_backend = "gloo"
+    device = torch.device("cpu")
+
+    def __init__(self, rank):
+        self.rank = rank
+
+    def open(self, cfg):
+        from paper_1501_03450_b200 import workloads as W
+        self.state = np.array(cfg["state"])
+        self.state[6:9] = 0.0
+        self.state[7] = 1.0 if self.rank == 0 else 0.5          # the ranks report different polarizations
+        self.state[8] = 0.0 if self.rank == 0 else 0.25
+        return W.steps_per_turn(cfg["lattice"], cfg["n_slices"])
+
+    def track(self, turns, split, n_slices, depth):
+        import time
+        time.sleep(0.02 * (self.rank + 1))                      # rank 1 is the slow one
+
+    def polarization(self):
+        p = self.state[6:9].mean(axis=1)
+        return np.append(p, np.linalg.norm(p)), 0
+
+    def track_host(self, turns, split, n_slices, depth):
+        self.track(turns, split, n_slices, depth)
+
+    def last_kernel(self):
+        return "stub"
+
+    def flush(self, k):
+        pass
+
+    def sync(self):
+        pass
+
+    def mark(self):
+        import time
+        return time.perf_counter()
+
+    @staticmethod
+    def ms_between(a, b):
+        return 1e3 * (b - a)
+
+    def clock_sampler(self):
+        return _StubSampler()
+
+    def roofline(self, cfg, n, turns, spt, kernel_ms):
+        return {"kernel_ms": kernel_ms}
+
+    def close(self):
+        pass
+
+
+def _bench_worker(rank, world, port, out):
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    sys.path.insert(0, root)
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world),
+                      LOCAL_RANK=str(rank))
+    import bench
+    args = bench.parse_args(["--gpus", "2", "--steps", "3", "--warmup", "1", "--config", "3", "--particles", "64",
+                             "--turns", "2", "--no-cpu-baseline"])
+    cfg = bench.configure(args)
+    seed0 = cfg["state"].copy()
+    line = bench.run_ours(args, cfg, _StubMachine(rank), args.config)
+    out.put((rank, line, bool(np.array_equal(seed0, cfg["state"]))))
+    dist.destroy_process_group()
+
+
+def test_bench_rank_shard_and_allreduce_path_on_two_gloo_ranks():
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_bench_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    got = dict((r, (line, same)) for r, line, same in (out.get(timeout=300) for _ in range(2)))
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    line, same0 = got[0]
+    assert got[1][0] is None and line is not None                # rank 0 alone reports
+    assert same0 and not got[1][1]                               # weak scaling: rank 1 drew its own bunch
+    assert line["n_gpus"] == 2 and line["scaling"] == "weak" and line["lost"] == 0
+    spt = line["config"]["steps_per_particle_turn"]
+    units = 2 * 64 * 2 * spt                                     # BOTH ranks' particles x turns x steps per turn
+    # the time is the slow rank's (max over ranks): 3 steps of >= 40 ms
+    assert line["ms_per_step"] >= 40.0 and line["ms_per_step"] < 400.0
+    assert abs(line["value"] - units / (line["ms_per_step"] * 1e-3)) < 1e-6 * line["value"]
+    assert abs(line["e2e"]["value"] / line["value"] - 1) < 0.5
+    # bunch-wide polarization = mean over both ranks' particles
+    assert np.allclose(line["polarization"][:3], [0.0, 0.75, 0.125], atol=1e-15)
+    assert abs(line["polarization"][3] - np.hypot(0.75, 0.125)) < 1e-15
