@@ -255,8 +255,7 @@ class CudaMachine:
         peak_meas, _ = self.diag.fp64_peak()
         peak_rrr, _ = self.diag.fp64_peak_rrr()
         kname = self.last_kernel()
-        chain = kname == "track_chain_kernel"
-        info = self.diag.kernel_info(split, depth, chain)
+        info = self.diag.kernel_info(split, depth, kname)
         roof = {"bound": "alu", "unit": "TFLOP/s",
                 "kernel": "gst::%s<%d,%d,%d>" % (kname, split % 3, depth, 4 if split >= 3 else 2),
                 "kernel_ms": kernel_ms, "kernel_info": info, "peak": peak_meas,

@@ -164,8 +164,11 @@ gst_status gst_track_pwc(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, 
  *                      bunch fits the chip in fewer than 1.5 waves but fills its sub-partitions unevenly (e.g. 65 536
  *                      particles = 3.46 warps each), the turns are cut into chunks and the warps of particles rotate
  *                      over all resident warp slots (csrc/track_chain_kernel.cuh, a cooperative launch)
- *   GST_LAUNCH_STATIC  never rotate: every warp keeps its slot for the whole call                                    */
-typedef enum { GST_LAUNCH_AUTO = 0, GST_LAUNCH_STATIC = 1 } gst_launch_mode;
+ *                      Bunches of at most two warps per sub-partition take a kernel variant compiled with registers to
+ *                      spare ("track_kernel_fat", see gst_bunch_last_kernel)
+ *   GST_LAUNCH_STATIC  never rotate: every warp keeps its slot for the whole call
+ *   GST_LAUNCH_LEAN    as GST_LAUNCH_STATIC, and always the occupancy-oriented kernel, whatever the bunch size        */
+typedef enum { GST_LAUNCH_AUTO = 0, GST_LAUNCH_STATIC = 1, GST_LAUNCH_LEAN = 2 } gst_launch_mode;
 gst_status gst_bunch_set_launch(gst_bunch* b, gst_launch_mode mode);
 
 /* Synchronise `cuda_stream` and report whether every gst_track enqueued on this bunch so far ran to the end:
@@ -181,8 +184,12 @@ gst_status gst_polarization(gst_bunch* b, void* cuda_stream, double out[4], int6
 /* Geometric rms emittances (a13; reading A19), HOST out = {eps_x, eps_y}; synchronises the stream. */
 gst_status gst_emittance(gst_bunch* b, void* cuda_stream, double out_exy[2]);
 
-/* Name of the kernel the last gst_track / gst_track_pwc on this bunch launched: "track_kernel" or
- * "track_chain_kernel" ("" before the first call).  Static storage.                                 */
+/* Name of the kernel the last gst_track / gst_track_pwc on this bunch launched ("" before the first call; static
+ * storage): "track_kernel"; "track_chain_kernel" (the rotating launch); "track_kernel_fat": the same code compiled
+ * with registers to spare, taken for bunches of at most two warps per SM sub-partition (37 888 particles on a B200),
+ * where one warp's dependency chains set the time -- the same source compiled a second time, so results agree
+ * with "track_kernel" to rounding (1e-13), not bit for bit; "track_chain_kernel" IS bit-identical to
+ * "track_kernel".                                                                                     */
 const char* gst_bunch_last_kernel(const gst_bunch* b);
 
 /* Copy the lost flags (1 = lost) to HOST memory, n bytes; synchronises the stream and reports a failed

@@ -466,7 +466,7 @@ gst_status gst_bunch_set_reference(gst_bunch* b, const gst_beam* beam, int64_t t
 }
 
 gst_status gst_bunch_set_launch(gst_bunch* b, gst_launch_mode mode) {
-  if (!b || (mode != GST_LAUNCH_AUTO && mode != GST_LAUNCH_STATIC)) return fail(GST_EINVAL, "null bunch or unknown launch mode %d", (int)mode);
+  if (!b || (mode != GST_LAUNCH_AUTO && mode != GST_LAUNCH_STATIC && mode != GST_LAUNCH_LEAN)) return fail(GST_EINVAL, "null bunch or unknown launch mode %d", (int)mode);
   b->launch_mode = mode;
   return GST_OK;
 }
@@ -521,6 +521,7 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   rq.steps_per_turn = gst_lattice_steps_per_turn(lat, table_slices);
   rq.sms = lat->sms;
   rq.allow_chain = b->launch_mode == GST_LAUNCH_AUTO;
+  rq.allow_fat = b->launch_mode != GST_LAUNCH_LEAN;
   rq.chain.scratch = b->d_chain;
   rq.chain.flag = b->d_chain + gst::CHAIN_SCRATCH_INTS;
   rq.chain.E0 = b->d_chain_E0;

@@ -181,7 +181,7 @@ __global__ void __launch_bounds__(TRACK_BLOCK, TRACK_MIN_BLOCKS) track_chain_ker
     ref.E0lo = k == 0 ? a.E0lo : __ldcg(ch.E0 + ch.n_chains + c);
     PCon pc;
     pcon_set(pc, z.Pt, ref, a.G);
-    typename SpinPolicy<DEPTH, SPLIT>::type spin(z);
+    typename SpinPolicy<DEPTH, SPLIT, false>::type spin(z);
     const long long t0 = k * ch.chunk_turns;
     const long long t1 = t0 + ch.chunk_turns < a.n_turns ? t0 + ch.chunk_turns : a.n_turns;
     const bool lost = track_turns<SPLIT, ORDER, false>(z, ref, pc, spin, t0, t1, a, smem_raw);

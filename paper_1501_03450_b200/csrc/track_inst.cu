@@ -48,33 +48,33 @@ cudaError_t GST_CAT4(launch_tu, GST_TU_SPLIT, GST_TU_GROUP)(int order, int depth
   }
 }
 
-cudaError_t GST_CAT4(kernel_info_tu, GST_TU_SPLIT, GST_TU_GROUP)(int order, int depth, bool chain, KernelInfo* out) {
+cudaError_t GST_CAT4(kernel_info_tu, GST_TU_SPLIT, GST_TU_GROUP)(int order, int depth, int variant, KernelInfo* out) {
   constexpr int S = GST_TU_SPLIT;
   (void)order;
   switch (depth) {
 #if GST_TU_GROUP == 0
 #ifndef GST_ONLY_DEPTH
-    case 0: return kernel_info<S, 0, 2>(chain, out);
-    case -1: return kernel_info<S, -1, 2>(chain, out);
+    case 0: return kernel_info<S, 0, 2>(variant, out);
+    case -1: return kernel_info<S, -1, 2>(variant, out);
 #endif
 #if !defined(GST_ONLY_DEPTH) || GST_ONLY_DEPTH <= 3
-    GST_CASE(1, 2) return kernel_info<S, 1, 2>(chain, out);
-    GST_CASE(2, 2) return kernel_info<S, 2, 2>(chain, out);
-    GST_CASE(3, 2) return kernel_info<S, 3, 2>(chain, out);
+    GST_CASE(1, 2) return kernel_info<S, 1, 2>(variant, out);
+    GST_CASE(2, 2) return kernel_info<S, 2, 2>(variant, out);
+    GST_CASE(3, 2) return kernel_info<S, 3, 2>(variant, out);
 #endif
 #elif GST_TU_GROUP == 1
 #if !defined(GST_ONLY_DEPTH) || GST_ONLY_DEPTH >= 4
-    GST_CASE(4, 2) return kernel_info<S, 4, 2>(chain, out);
-    GST_CASE(5, 2) return kernel_info<S, 5, 2>(chain, out);
-    GST_CASE(6, 2) return kernel_info<S, 6, 2>(chain, out);
+    GST_CASE(4, 2) return kernel_info<S, 4, 2>(variant, out);
+    GST_CASE(5, 2) return kernel_info<S, 5, 2>(variant, out);
+    GST_CASE(6, 2) return kernel_info<S, 6, 2>(variant, out);
 #endif
 #elif !defined(GST_ONLY_DEPTH)
-    case 1: return kernel_info<S, 1, 4>(chain, out);
-    case 2: return kernel_info<S, 2, 4>(chain, out);
-    case 3: return kernel_info<S, 3, 4>(chain, out);
-    case 4: return kernel_info<S, 4, 4>(chain, out);
-    case 5: return kernel_info<S, 5, 4>(chain, out);
-    case 6: return kernel_info<S, 6, 4>(chain, out);
+    case 1: return kernel_info<S, 1, 4>(variant, out);
+    case 2: return kernel_info<S, 2, 4>(variant, out);
+    case 3: return kernel_info<S, 3, 4>(variant, out);
+    case 4: return kernel_info<S, 4, 4>(variant, out);
+    case 5: return kernel_info<S, 5, 4>(variant, out);
+    case 6: return kernel_info<S, 6, 4>(variant, out);
 #endif
     default: return cudaErrorNotSupported;
   }

@@ -489,9 +489,11 @@ template <int KIND> struct MidSpin {
   }
   __device__ __forceinline__ void snake(const Quat& q) { quat_rotate(q, Sx, Sy, Ss); }
 };
-template <int DEPTH, int SPLIT> struct SpinPolicy { using type = FusedSpin<DEPTH, SPLIT == SPLIT_MK>; };
-template <int SPLIT> struct SpinPolicy<0, SPLIT> { using type = MidSpin<0>; };
-template <int SPLIT> struct SpinPolicy<-1, SPLIT> { using type = MidSpin<-1>; };
+// FAT: the kernel variant for bunches that leave most of the chip empty (see track_kernel below); there the matrix-kick
+// loops keep their two-edge bodies.
+template <int DEPTH, int SPLIT, bool FAT> struct SpinPolicy { using type = FusedSpin<DEPTH, SPLIT == SPLIT_MK && !FAT>; };
+template <int SPLIT, bool FAT> struct SpinPolicy<0, SPLIT, FAT> { using type = MidSpin<0>; };
+template <int SPLIT, bool FAT> struct SpinPolicy<-1, SPLIT, FAT> { using type = MidSpin<-1>; };
 
 // a4: exact sector bend (10), spin from the slice-edge Omega (6b).
 // With c = cos(h ds), s = sin(h ds), A = sqrt(Pa^2 - Px^2), g = A - eta(1 + hX):
@@ -1167,7 +1169,14 @@ constexpr int TRACK_MIN_BLOCKS = 8;
 // The fourth-order matrix-kick map carries two tables of linear-flow coefficients: at 128 registers it spills
 // 800 B per thread.  With 6 blocks per SM (3 warps per sub-partition, 167 registers, no spills) it measured 20 %
 // faster; every other instantiation is equal or slightly slower that way (profiles/r01_notes.md).
-__host__ __device__ constexpr int track_min_blocks(int split, int order) { return (split == SPLIT_MK && order == 4) ? 6 : TRACK_MIN_BLOCKS; }
+// A bunch of at most two warps per sub-partition is not short of registers but of parallelism: one warp's dependency
+// chains set the time.  The FAT variant is compiled for 4 blocks per SM (up to 255 registers; ptxas takes 170-190, no
+// spills, more of the loop bodies in flight): measured +7 % (bend-kick) to +18 % (matrix-kick, with its two-edge loop
+// bodies) on 4096-particle bunches, +7 % at 16 384.
+constexpr int TRACK_FAT_BLOCKS = 4;
+__host__ __device__ constexpr int track_min_blocks(int split, int order, bool fat) {
+  return fat ? TRACK_FAT_BLOCKS : (split == SPLIT_MK && order == 4) ? 6 : TRACK_MIN_BLOCKS;
+}
 
 // a0: the lattice is ALWAYS read from shared memory (LDS; element records and sequence entries through a pointer that
 // may point to global or shared memory measured 3 % slower).  Two layouts of the dynamic shared memory, chosen on the
@@ -1251,8 +1260,8 @@ __device__ __forceinline__ bool track_turns(State& z, Ref& ref, PCon& pc, Spin& 
   return lost;
 }
 
-template <int SPLIT, int DEPTH, int ORDER, bool STREAMED>
-__global__ void __launch_bounds__(TRACK_BLOCK, track_min_blocks(SPLIT, ORDER)) track_kernel(const TrackArgs a) {
+template <int SPLIT, int DEPTH, int ORDER, bool STREAMED, bool FAT>
+__global__ void __launch_bounds__(TRACK_BLOCK, track_min_blocks(SPLIT, ORDER, FAT)) track_kernel(const TrackArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   stage_lattice<STREAMED>(a, smem_raw);
   if (*a.err != 0) return;                               // an earlier launch on this bunch failed: leave everything (gst.h)
@@ -1271,7 +1280,7 @@ __global__ void __launch_bounds__(TRACK_BLOCK, track_min_blocks(SPLIT, ORDER)) t
   ref.E0lo = a.E0lo;
   PCon pc;
   pcon_set(pc, z.Pt, ref, a.G);
-  typename SpinPolicy<DEPTH, SPLIT>::type spin(z);
+  typename SpinPolicy<DEPTH, SPLIT, FAT>::type spin(z);
   const bool lost = track_turns<SPLIT, ORDER, STREAMED>(z, ref, pc, spin, 0, a.n_turns, a, smem_raw);
   if (!valid) return;
   if (lost) { a.lost[j] = 1; return; }

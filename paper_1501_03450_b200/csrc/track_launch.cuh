@@ -18,6 +18,7 @@ struct LaunchRequest {
   long long steps_per_turn = 1;
   int sms = 0;                  // SMs of the bunch's device
   bool allow_chain = false;     // GST_LAUNCH_AUTO: the planner may take the rotating launch
+  bool allow_fat = true;        // not GST_LAUNCH_LEAN: small bunches take the variant with registers to spare
   ChainArgs chain;              // the bunch's scratch for it (n_chains, chunk_turns, poll_limit are filled in here)
   long long poll_limit_override = 0;   // != 0: fault injection (include/gst_diag.h)
   const char* kernel = "";      // out: name of the kernel launched
@@ -33,7 +34,7 @@ struct KernelInfo { int registers = 0, local_bytes = 0, blocks_per_sm = 0; };
 // depth >= 1: Romberg depth, 0 / -1: mid-slice PWC orderings.
 #define GST_DECLARE_TU(S, G)                                                                        \
   cudaError_t launch_tu_##S##_##G(int order, int depth, LaunchRequest& rq, cudaStream_t st);         \
-  cudaError_t kernel_info_tu_##S##_##G(int order, int depth, bool chain, KernelInfo* out);
+  cudaError_t kernel_info_tu_##S##_##G(int order, int depth, int variant, KernelInfo* out);
 GST_DECLARE_TU(0, 0) GST_DECLARE_TU(0, 1) GST_DECLARE_TU(0, 2)
 GST_DECLARE_TU(1, 0) GST_DECLARE_TU(1, 1) GST_DECLARE_TU(1, 2)
 GST_DECLARE_TU(2, 0) GST_DECLARE_TU(2, 1) GST_DECLARE_TU(2, 2)
@@ -56,8 +57,9 @@ inline int tu_group(int order, int depth) { return order == 4 ? 2 : (depth >= 4 
 inline cudaError_t launch_tracking(int split3, int order, int depth, LaunchRequest& rq, cudaStream_t st) {
   GST_DISPATCH_TU(launch_tu, order, depth, rq, st)
 }
-inline cudaError_t kernel_info_of(int split3, int order, int depth, bool chain, KernelInfo* out) {
-  GST_DISPATCH_TU(kernel_info_tu, order, depth, chain, out)
+// variant: 0 = track_kernel, 1 = track_chain_kernel, 2 = track_kernel (FAT)
+inline cudaError_t kernel_info_of(int split3, int order, int depth, int variant, KernelInfo* out) {
+  GST_DISPATCH_TU(kernel_info_tu, order, depth, variant, out)
 }
 #undef GST_DISPATCH_TU
 
@@ -137,18 +139,23 @@ cudaError_t launch_track(LaunchRequest& rq, cudaStream_t st) {
     }
   }
   // T1: one thread per particle; shared memory kept small so that 8 blocks of 64 threads stay resident
-  auto kern = p.streamed ? track_kernel<SPLIT, DEPTH, ORDER, true> : track_kernel<SPLIT, DEPTH, ORDER, false>;
+  // at most two warps per sub-partition: the variant with registers to spare (track_kernel.cuh: FAT)
+  const bool fat = rq.allow_fat && !p.streamed && (a.n + 31) / 32 <= 2LL * 4 * rq.sms;
+  auto kern = p.streamed ? track_kernel<SPLIT, DEPTH, ORDER, true, false>
+              : fat      ? track_kernel<SPLIT, DEPTH, ORDER, false, true>
+                         : track_kernel<SPLIT, DEPTH, ORDER, false, false>;
   const unsigned blocks = (unsigned)((a.n + TRACK_BLOCK - 1) / TRACK_BLOCK);
   kern<<<blocks, TRACK_BLOCK, p.bytes, st>>>(a);
-  rq.kernel = "track_kernel";
+  rq.kernel = fat ? "track_kernel_fat" : "track_kernel";
   return cudaGetLastError();
 }
 
 template <int SPLIT, int DEPTH, int ORDER>
-cudaError_t kernel_info(bool chain, KernelInfo* out) {
-  const void* f = (const void*)track_kernel<SPLIT, DEPTH, ORDER, false>;
+cudaError_t kernel_info(int variant, KernelInfo* out) {
+  const void* f = variant == 2 ? (const void*)track_kernel<SPLIT, DEPTH, ORDER, false, true>
+                               : (const void*)track_kernel<SPLIT, DEPTH, ORDER, false, false>;
   if constexpr (ORDER == 2 && DEPTH >= 1) {
-    if (chain) f = (const void*)track_chain_kernel<SPLIT, DEPTH, ORDER>;
+    if (variant == 1) f = (const void*)track_chain_kernel<SPLIT, DEPTH, ORDER>;
   }
   cudaFuncAttributes at;
   cudaError_t e = cudaFuncGetAttributes(&at, f);

@@ -40,7 +40,7 @@ EXPORTS = ["gst_lattice_create", "gst_lattice_destroy", "gst_lattice_steps_per_t
            "gst_bunch_destroy", "gst_track", "gst_polarization", "gst_emittance", "gst_bunch_lost",
            "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host", "gst_last_error",
            "gst_bunch_set_launch", "gst_bunch_status", "gst_track_pwc", "gst_bunch_last_kernel"]
-LAUNCH_AUTO, LAUNCH_STATIC = 0, 1
+LAUNCH_AUTO, LAUNCH_STATIC, LAUNCH_LEAN = 0, 1, 2
 
 
 def lib():
@@ -186,7 +186,8 @@ class Bunch:
         return lib().gst_bunch_last_kernel(self._h).decode()
 
     def set_launch(self, mode):
-        """gst_bunch_set_launch: LAUNCH_AUTO (default) or LAUNCH_STATIC (never the rotating launch)."""
+        """gst_bunch_set_launch: LAUNCH_AUTO (default), LAUNCH_STATIC (never the rotating launch) or LAUNCH_LEAN (nor the
+        small-bunch kernel variant)."""
         _check(lib().gst_bunch_set_launch(self._h, int(mode)))
 
     def status(self, stream=None):

@@ -55,8 +55,11 @@ def chain_poll_limit(bunch, polls):
     gst._check(lib().gst_diag_chain_poll_limit(bunch._h, int(polls)))
 
 
-def kernel_info(split, depth, chain=False):
+KERNEL_VARIANTS = {"track_kernel": 0, "track_chain_kernel": 1, "track_kernel_fat": 2}
+
+
+def kernel_info(split, depth, kernel="track_kernel"):
     """gst_diag_kernel_info: {registers, local_bytes, blocks_per_sm} of one tracking-kernel instantiation."""
     r, l, b = C.c_int(0), C.c_int(0), C.c_int(0)
-    gst._check(lib().gst_diag_kernel_info(int(split), int(depth), 1 if chain else 0, C.byref(r), C.byref(l), C.byref(b)))
+    gst._check(lib().gst_diag_kernel_info(int(split), int(depth), KERNEL_VARIANTS[kernel], C.byref(r), C.byref(l), C.byref(b)))
     return {"registers": r.value, "local_bytes": l.value, "blocks_per_sm": b.value}

@@ -37,13 +37,14 @@ def O():
     return oracle
 
 
-def gpu_track(gst, lat, beam, state, n_turns, split, n_slices, depth, chunks=None, static=False, want_kernel=None):
+def gpu_track(gst, lat, beam, state, n_turns, split, n_slices, depth, chunks=None, static=False, want_kernel=None,
+              lean=False):
     """depth >= 1: gst_track; depth = W.PWC_HALF_SLICE / W.PWC_DKSKD (0 / -1): gst_track_pwc"""
     L = gst.Lattice(lat, beam)
     d = torch.tensor(state, dtype=torch.float64, device="cuda").contiguous()
     b = gst.Bunch(d)
-    if static:
-        b.set_launch(gst.LAUNCH_STATIC)
+    if static or lean:
+        b.set_launch(gst.LAUNCH_LEAN if lean else gst.LAUNCH_STATIC)
     for nt in (chunks or [n_turns]):
         if depth >= 1:
             b.track(L, nt, split, n_slices, depth)
@@ -125,12 +126,17 @@ def test_all_splits_depths_all_element_types(gst, O, split, depth, n_slices):
     n = 200                                   # 3 full blocks of 64 and a ragged tail of 8
     st = W.gaussian_bunch(7, n, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
     ref, rlost, g_ref = O.track(lat, bm, st, 2, split, n_slices, depth)
-    got, lost, pol, emit, g_gpu = gpu_track(gst, lat, bm, st, 2, split, n_slices, depth)
+    # 200 particles take the small-bunch kernel variant; the variant large bunches get must give the same
+    got, lost, pol, emit, g_gpu = gpu_track(gst, lat, bm, st, 2, split, n_slices, depth, want_kernel="track_kernel_fat")
+    lean = gpu_track(gst, lat, bm, st, 2, split, n_slices, depth, lean=True, want_kernel="track_kernel")
     assert not rlost.any() and not lost.any()
     assert orbit_err(got, ref) < 2e-12, orbit_err(got, ref)
     assert spin_err(got, ref) < 2e-12, spin_err(got, ref)
     assert abs(g_gpu - g_ref) < 1e-12 * g_ref
     assert np.max(np.abs(np.linalg.norm(got[6:9], axis=0) - 1)) < 1e-12     # A9: |S| = 1 without renormalising
+    assert orbit_err(lean[0], ref) < 2e-12 and spin_err(lean[0], ref) < 2e-12 and lean[4] == g_gpu
+    # the same source compiled twice: the two differ by the compiler's choice of fused multiply-adds only
+    assert orbit_err(lean[0], got) < 1e-13 and spin_err(lean[0], got) < 1e-13
 
 
 @pytest.mark.parametrize("split", [W.SPLIT_DRIFT_KICK_4, W.SPLIT_BEND_KICK_4, W.SPLIT_MATRIX_KICK_4])
