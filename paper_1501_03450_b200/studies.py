@@ -1,10 +1,9 @@
-"""The two BASELINE studies that are more than one timed launch, run through the C ABI on one GPU.
+"""The two BASELINE studies that are more than one timed launch, and the paper's single-element study, run through the
+C ABI on one GPU.
 
     python -m paper_1501_03450_b200.studies ramp  [--particles N] [--turns T] [--chunk 100] [--out FILE.md]
     python -m paper_1501_03450_b200.studies sweep [--particles N] [--turns T] [--out FILE.md]
     python -m paper_1501_03450_b200.studies fig7  [--out FILE.md]
-    python -m paper_1501_03450_b200.studies fig14 [--particles N] [--out FILE.md]
-    python -m paper_1501_03450_b200.studies crossing [--out FILE.md]
 
 ramp  : BASELINE configs[3] (SURVEY config 4): the RHIC-like ring with its cavity ramping the energy by
         100 keV/turn from G*gamma = 45.0, 2^20 particles, 5000 turns; the bunch polarization, emittances
@@ -20,16 +19,6 @@ fig7  : the paper's single-element study (Fig. 7): spin error of its 
         across the RHIC IR quadrupole (1.83 m, 70 T/m), arc dipole (9.45 m, 2.225 deg) and the 1.3 T,
         2.1 m solenoid at 200 GeV and at 1.2 GeV, against the number of slices, for mid-slice PWC
         and for k = 0..3 Romberg iterations on the edge scheme; reference = 256 slices, k = 3.
-
-fig14 : the paper's single-turn spin-error study (Fig. 14) on the synthetic ring of config 5: error (46) after
-        ONE turn against the number of slices, no Romberg, for the PWC integrators the caption names -- DKSKD and
-        DKDSDKD on drift-kick orbits, DKDSDKD on bend-kick/matrix-kick orbits -- and for the trapezoid edge product;
-        reference = matrix-kick, 256 slices, three Romberg iterations.
-
-crossing : the ramp (A13) against a closed form: an on-axis particle is accelerated through an isolated resonance of known
-        strength (a partial snake of angle 2 pi eps in a planar ring: tune gap eps at integer G*gamma,
-        workloads.resonance_crossing_ring) from G*gamma = 44.5 to 45.5 at several rates; the final vertical spin is set
-        against the Froissart-Stora formula 2 exp(-pi eps^2 / (2 alpha)) - 1, alpha = d(G gamma)/d(theta).
 
 Every number of the hot path comes from the CUDA kernels; torch is used for device memory, the error
 norms of the report and nothing else.  One JSON line per report row on stdout; --out adds a markdown table.
@@ -219,89 +208,6 @@ def fig7(args):
                 f.write("\n")
 
 
-def fig14(args):
-    import torch
-    from . import gst
-    cfg = W.config(5, n_particles=args.particles or 65536, n_turns=1)
-    n = cfg["state"].shape[1]
-    lat = gst.Lattice(cfg["lattice"], cfg["beam"])
-    init = _device_state(torch, cfg["state"])
-
-    def run(split, n_slices, depth):
-        dev = init.clone()
-        b = gst.Bunch(dev)
-        if depth >= 1:
-            b.track(lat, 1, split, n_slices, depth)
-        else:
-            b.track_pwc(lat, 1, split, n_slices, depth)
-        torch.cuda.synchronize()
-        b.close()
-        return dev
-    ref = run(W.SPLIT_MATRIX_KICK, 256, 4)
-    curves = [("DKSKD, drift-kick", W.SPLIT_DRIFT_KICK, W.PWC_DKSKD), ("DKDSDKD, drift-kick", W.SPLIT_DRIFT_KICK, W.PWC_HALF_SLICE),
-              ("DKDSDKD, matrix-kick", W.SPLIT_MATRIX_KICK, W.PWC_HALF_SLICE), ("edge product k=0, drift-kick", W.SPLIT_DRIFT_KICK, 1),
-              ("edge product k=0, matrix-kick", W.SPLIT_MATRIX_KICK, 1)]
-    slices = [1, 2, 4, 8, 16, 32, 64]
-    table = {}
-    for name, split, depth in curves:
-        for ns in slices:
-            dev = run(split, ns, depth)
-            err = torch.linalg.vector_norm(dev[6:9] - ref[6:9], dim=0).mean().item()        # (46) P:733
-            table[name, ns] = err
-            print(json.dumps(dict(curve=name, slices=ns, spin_err=err)))
-    if args.out:
-        with open(args.out, "w") as f:
-            f.write("# Single-turn spin error (46) against the number of slices, no Romberg (the paper's Fig. 14, P:731-748)\n\n")
-            f.write("Command: `python -m paper_1501_03450_b200.studies fig14 --particles %d`\n\n" % n)
-            f.write("Config-5 ring (RHIC-like, no snakes), %d particles, one turn; reference: matrix-kick, 256 slices, k = 3 (P:736).\n\n" % n)
-            f.write("| slices | " + " | ".join(c[0] for c in curves) + " |\n|---|" + "---|" * len(curves) + "\n")
-            for ns in slices:
-                f.write("| %d | " % ns + " | ".join("%.2e" % table[c[0], ns] for c in curves) + " |\n")
-    lat.close()
-
-
-def crossing(args):
-    import math
-    import torch
-    from . import gst
-    rows = []
-    for dGg in (1e-3, 2.5e-4, 1e-4):
-        for x in (0.05, 0.2, 0.5, math.log(2.0), 1.0, 2.0, 4.0):        # x = pi eps^2 / (2 alpha)
-            eps = math.sqrt(x * dGg) / math.pi
-            lat_e, beam, turns = W.resonance_crossing_ring(dGg, eps)
-            lat = gst.Lattice(lat_e, beam)
-            st = np.zeros((9, 32))
-            st[7] = 1.0
-            dev = _device_state(torch, st)
-            b = gst.Bunch(dev)
-            ms = _timed_track(torch, b, lat, turns, W.SPLIT_BEND_KICK, 4, 3)
-            pol, _ = b.polarization()
-            g1, _ = b.reference()
-            b.close()
-            lat.close()
-            fs = 2.0 * math.exp(-x) - 1.0
-            row = dict(dGg_per_turn=dGg, eps=eps, turns=turns, x=x, Sy=pol[1], froissart_stora=fs, diff=pol[1] - fs,
-                       nutation_bound=2.0 * eps, Ggamma_end=G_PROTON * g1, ms=ms)
-            rows.append(row)
-            print(json.dumps(row))
-    if args.out:
-        with open(args.out, "w") as f:
-            f.write("# Ramp through an isolated spin resonance against the Froissart-Stora formula\n\n")
-            f.write("Command: `python -m paper_1501_03450_b200.studies crossing --out %s`\n\n" % args.out)
-            f.write("16-cell FODO ring, partial snake of angle 2 pi eps (tune gap eps at G*gamma = 45), cavity adding dGg to "
-                    "G*gamma_o per turn (A13), on-axis particles, bend-kick, 4 slices, depth 3, G*gamma 44.5 -> 45.5.  "
-                    "x = pi eps^2 / (2 alpha) = pi^2 eps^2 / dGg; Froissart-Stora: Sy = 2 exp(-x) - 1.  The run starts and ends "
-                    "half a unit of tune from the resonance, where the stable spin direction is tilted by about 2 eps from the "
-                    "vertical: the difference from the asymptotic formula is a few eps and falls in proportion to eps at "
-                    "fixed x (compare the three blocks).\n\n")
-            f.write("| dGg per turn | turns | eps | x | Sy (CUDA path) | Froissart-Stora | diff | 2 eps | G*gamma at the end |\n")
-            f.write("|---|---|---|---|---|---|---|---|---|\n")
-            for r in rows:
-                f.write("| %.1e | %d | %.4e | %.3f | %+.5f | %+.5f | %+.1e | %.1e | %.9f |\n" % (
-                    r["dGg_per_turn"], r["turns"], r["eps"], r["x"], r["Sy"], r["froissart_stora"], r["diff"],
-                    r["nutation_bound"], r["Ggamma_end"]))
-
-
 def main(argv=None):
     ap = argparse.ArgumentParser(description=__doc__, formatter_class=argparse.RawDescriptionHelpFormatter)
     sub = ap.add_subparsers(dest="study", required=True)
@@ -320,14 +226,9 @@ def main(argv=None):
     s.add_argument("--out", default=None)
     g = sub.add_parser("fig7")
     g.add_argument("--out", default=None)
-    h = sub.add_parser("fig14")
-    h.add_argument("--particles", type=int, default=None)
-    h.add_argument("--out", default=None)
-    x = sub.add_parser("crossing")
-    x.add_argument("--out", default=None)
     args = ap.parse_args(argv)
     t0 = time.time()
-    {"ramp": ramp, "sweep": sweep, "fig7": fig7, "fig14": fig14, "crossing": crossing}[args.study](args)
+    {"ramp": ramp, "sweep": sweep, "fig7": fig7}[args.study](args)
     print(json.dumps(dict(wall_s=time.time() - t0)))
 
 
