@@ -16,8 +16,9 @@ stands) on the host cores on a bounded sample of the same workload.
 
 The roofline fraction needs the number of fp64 flops the kernel EXECUTES per particle-turn, which only ncu can count:
 flop_model.json (written by flop_model.py from committed ncu captures under profiles/) holds it per instantiation,
-together with the registers and stack frame of the kernel that was captured.  `frac` is printed only when the loaded
-library's kernel still has those resources; otherwise it is null and the line says why.
+together with the registers and stack frame of the kernel that was captured and the fingerprint of the kernel sources
+it was compiled from.  `frac` is printed only when the loaded library's kernel has the same; otherwise it is null and the
+line says why (re-capture: see flop_model.py).
 """
 import argparse
 import json
@@ -255,7 +256,7 @@ class CudaMachine:
         peak_meas, _ = self.diag.fp64_peak()
         peak_rrr, _ = self.diag.fp64_peak_rrr()
         kname = self.last_kernel()
-        info = self.diag.kernel_info(split, depth, kname)
+        info = dict(self.diag.kernel_info(split, depth, kname), source_hash=self.diag.kernel_source_hash())
         roof = {"bound": "alu", "unit": "TFLOP/s",
                 "kernel": "gst::%s<%d,%d,%d>" % (kname, split % 3, depth, 4 if split >= 3 else 2),
                 "kernel_ms": kernel_ms, "kernel_info": info, "peak": peak_meas,

@@ -6,7 +6,7 @@ One capture = two files made by the SAME bench.py command on the GPU box, first 
     ncu --clock-control none -k regex:track_ -c 1 --csv --metrics METRICS --log-file gpurun_out/fm_TAG.csv \
         python bench.py ARGS --steps 1 --warmup 0 --turns 16 --no-e2e --no-cpu-baseline
 
-(METRICS below.)  Then, here:   python flop_model.py profiles/r02_fm_TAG.csv [more .csv ...]
+(METRICS below.)  Then, here:   python flop_model.py [--source-hash H] profiles/r02_fm_TAG.csv [more .csv ...]
 Each .csv needs its .json beside it: the JSON line names the workload, the kernel that ran and its registers and
 stack frame (gst_diag_kernel_info), which bench.py later compares with the loaded library before it prints a fraction.
 
@@ -76,7 +76,7 @@ def to_float(v, u):
     return x * scale.get(u, 1)
 
 
-def entry_from(csv_path):
+def entry_from(csv_path, source_hash=None):
     line = None
     for ln in open(os.path.splitext(csv_path)[0] + ".json"):
         if ln.startswith("{"):
@@ -89,6 +89,11 @@ def entry_from(csv_path):
     flop = 2 * got["dfma"] + got["dadd"] + got["dmul"]
     pt = particles * turns
     kname = roof["kernel"].split("::")[1].split("<")[0]
+    info = dict(roof["kernel_info"])
+    if "source_hash" not in info:      # a line printed before bench.py carried the fingerprint: name it on the command line
+        if not source_hash:
+            raise SystemExit("%s: no kernel source fingerprint in the bench line; pass --source-hash" % csv_path)
+        info["source_hash"] = source_hash
     return key, {
         "flop_per_particle_turn": flop / pt,
         "dfma_per_particle_turn": got["dfma"] / pt, "dadd_per_particle_turn": got["dadd"] / pt,
@@ -97,7 +102,7 @@ def entry_from(csv_path):
         "warp_inst_per_warp_turn": got.get("inst_executed", 0) / (pt / 32.0),
         "dram_bytes_per_launch": got.get("dram_read", 0) + got.get("dram_write", 0),
         "capture": {"particles": particles, "turns": turns, "duration_ms": got.get("duration_ns", 0) / 1e6,
-                    "kernel": kname, "kernel_info": roof["kernel_info"],
+                    "kernel": kname, "kernel_info": info,
                     "registers_per_thread": got.get("regs"), "fp64_pipe_pct_of_peak": got.get("fp64_pipe_pct"),
                     "issue_active_pct": got.get("issue_pct"), "warps_active_pct": got.get("warps_active_pct"),
                     "spill_instructions": got.get("spill_inst"), "branch_instructions": got.get("branches")},
@@ -107,8 +112,14 @@ def entry_from(csv_path):
 
 def main():
     model = json.load(open(OUT)) if os.path.exists(OUT) else {}
-    for path in sys.argv[1:]:
-        key, entry = entry_from(path)
+    args = sys.argv[1:]
+    source_hash = None
+    if "--source-hash" in args:
+        k = args.index("--source-hash")
+        source_hash = args[k + 1]
+        del args[k:k + 2]
+    for path in args:
+        key, entry = entry_from(path, source_hash)
         model[key] = entry
         print(key, "%.0f flop/particle-turn, %.0f fp64 instructions, kernel %s %s"
               % (entry["flop_per_particle_turn"], entry["fp64_inst_per_particle_turn"], entry["capture"]["kernel"],

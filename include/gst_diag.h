@@ -40,6 +40,11 @@ gst_status gst_diag_chain_poll_limit(gst_bunch* b, int64_t polls);
 gst_status gst_diag_kernel_info(gst_split split, int romberg_depth, int variant, int* out_registers,
                                 int* out_local_bytes, int* out_max_blocks_per_sm);
 
+/* Fingerprint (16 hex digits) of the sources and compiler flags the tracking kernels of this library were built
+ * from, as computed by paper_1501_03450_b200/build.py; "unknown" for a library built some other way.  bench.py prints
+ * a roofline fraction only when it equals the fingerprint stored with the ncu capture of the flop count.  Static.  */
+const char* gst_diag_kernel_source_hash(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -24,6 +24,19 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "-Xcompiler", "-fPIC"]
 
 
+KERNEL_SOURCES = ("track_kernel.cuh", "track_chain_kernel.cuh", "track_launch.cuh", "track_inst.cu")
+
+
+def kernel_source_hash() -> str:
+    """Fingerprint of what the tracking kernels are compiled from (sources and flags): compiled into the library
+    (gst_diag_kernel_source_hash) so that bench.py can tell whether its flop model was captured on this code."""
+    import hashlib
+    h = hashlib.sha1(" ".join(NVCC_FLAGS).encode())
+    for f in KERNEL_SOURCES:
+        h.update(open(os.path.join(CSRC, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     newest = max(os.path.getmtime(p) for p in DEPS)
     if not force and os.path.exists(OUT) and os.path.getmtime(OUT) >= newest:
@@ -36,6 +49,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         while pending and len(running) < workers:
             name, src, defs = pending.pop(0)
             obj = os.path.join(OBJ, name + ".o")
+            if name == "gst_diag":
+                defs = defs + ['-DGST_KERNEL_SOURCE_HASH="%s"' % kernel_source_hash()]
             cmd = [nvcc] + NVCC_FLAGS + defs + (["-Xptxas", "-v"] if verbose else []) + ["-c", "-o", obj, os.path.join(CSRC, src)]
             running.append((obj, cmd, subprocess.Popen(cmd, cwd=CSRC, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
         obj, cmd, proc = running.pop(0)

@@ -134,6 +134,11 @@ gst_status gst_diag_selftest_math(double out[2]) {
   return GST_OK;
 }
 
+#ifndef GST_KERNEL_SOURCE_HASH
+#define GST_KERNEL_SOURCE_HASH "unknown"
+#endif
+const char* gst_diag_kernel_source_hash(void) { return GST_KERNEL_SOURCE_HASH; }
+
 gst_status gst_diag_kernel_info(gst_split split, int romberg_depth, int variant, int* out_registers, int* out_local_bytes,
                                 int* out_max_blocks_per_sm) {
   if ((int)split < 0 || (int)split > 5 || romberg_depth < 1 || romberg_depth > 6) return fail(GST_EINVAL, "unknown split or depth");

@@ -6,7 +6,7 @@ import ctypes as C
 from . import gst
 
 EXPORTS = ["gst_diag_fp64_peak", "gst_diag_fp64_peak_rrr", "gst_diag_selftest_math", "gst_diag_chain_poll_limit",
-           "gst_diag_kernel_info"]
+           "gst_diag_kernel_info", "gst_diag_kernel_source_hash"]
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int)
 _ready = False
@@ -23,6 +23,8 @@ def lib():
         L.gst_diag_kernel_info.argtypes = [C.c_int, C.c_int, C.c_int, _ip, _ip, _ip]
         for name in EXPORTS:
             getattr(L, name).restype = C.c_int
+        L.gst_diag_kernel_source_hash.restype = C.c_char_p
+        L.gst_diag_kernel_source_hash.argtypes = []
         _ready = True
     return L
 
@@ -53,6 +55,11 @@ def selftest_math():
 def chain_poll_limit(bunch, polls):
     """gst_diag_chain_poll_limit: make the next rotating launches on `bunch` give up after `polls` polls (0: default)."""
     gst._check(lib().gst_diag_chain_poll_limit(bunch._h, int(polls)))
+
+
+def kernel_source_hash():
+    """gst_diag_kernel_source_hash: fingerprint of the kernel sources and flags this library was built from."""
+    return lib().gst_diag_kernel_source_hash().decode()
 
 
 KERNEL_VARIANTS = {"track_kernel": 0, "track_chain_kernel": 1, "track_kernel_fat": 2}
