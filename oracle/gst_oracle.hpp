@@ -18,10 +18,12 @@
 //   * in __float128       (ground truth for the cancellation checks),
 //   * in Dual<6>          (forward-mode derivatives -> Jacobians for symplecticity / optics pins).
 //
-// Parity status: every function here is pinned by tests/test_oracle_*.py EXCEPT the RF cavity
-// with ramp (rf_cavity, A12/A13) whose formulas are not in the paper: it is pinned only by the
-// small-amplitude synchrotron tune, the adiabatic invariants (transverse and longitudinal) and the
-// Froissart-Stora crossing of a partial-snake resonance; beyond that it is "parity unpinned".
+// Parity status: every function here is pinned by tests/test_oracle_*.py.  The RF cavity with ramp
+// (A12/A13) is a READING -- its formulas are not in the paper -- pinned by its linearised kick and the
+// one-turn longitudinal map at two energies, the re-referencing element by element, the adiabatic
+// invariants (transverse and longitudinal) and the Froissart-Stora crossing of a partial-snake
+// resonance (tests/test_oracle_rf_reductions.py); the config-4 polarization curve of a real lattice
+// has no closed form and is GPU-vs-oracle only.
 #pragma once
 #include <cmath>
 #include <cstdint>
