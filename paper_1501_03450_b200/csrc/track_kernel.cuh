@@ -378,9 +378,7 @@ template <int DEPTH> struct SpinAcc {
   // Q[l] holds step h*2^l, i.e. column entry k = DEPTH-1-l of (38).
   // The normalisation is a common positive factor, so the weights are taken relative to the finest level's (its
   // product enters with weight one) and the rotation divides by |q|^2 instead of normalising q first: a reciprocal
-  // instead of a reciprocal square root and eight multiplications less per element.  NORMALISE_FIRST keeps the
-  // reciprocal square root: in the rolled matrix-kick kernels that measured 4 % faster (0.5 % slower in the others).
-  template <bool NORMALISE_FIRST>
+  // instead of a reciprocal square root and eight multiplications less per element.
   __device__ __forceinline__ void finish(double& Sx, double& Sy, double& Ss) {
     Quat q = Q[0];
 #pragma unroll
@@ -388,13 +386,7 @@ template <int DEPTH> struct SpinAcc {
       q.w = fma(ROMBERG_REL[DEPTH - 1][l], Q[l].w, q.w); q.x = fma(ROMBERG_REL[DEPTH - 1][l], Q[l].x, q.x);
       q.y = fma(ROMBERG_REL[DEPTH - 1][l], Q[l].y, q.y); q.s = fma(ROMBERG_REL[DEPTH - 1][l], Q[l].s, q.s);
     }
-    if (NORMALISE_FIRST) {
-      const double rn = rsqrt_nr(fma(q.w, q.w, fma(q.x, q.x, fma(q.y, q.y, q.s * q.s))));
-      q.w *= rn; q.x *= rn; q.y *= rn; q.s *= rn;
-      quat_rotate(q, Sx, Sy, Ss);
-    } else {
-      quat_rotate_unnormalised(q, Sx, Sy, Ss);
-    }
+    quat_rotate_unnormalised(q, Sx, Sy, Ss);
   }
 };
 
@@ -447,15 +439,16 @@ __device__ __forceinline__ bool drift(State& z, double L, const PCon& c, const R
 //   FusedSpin<DEPTH>  -- the trapezoid / Romberg scheme (38)(39): every edge is folded into DEPTH level products
 //   MidSpin<KIND>     -- the mid-slice comparison integrators (37)
 // ROLLED: the matrix-kick kernels take the edges one per iteration with the level membership tested at run time
-// (uniform branches).  Their two-edge loop body would be 6.4 kB for the quadrupole (160 fp64 instructions per
-// slice), more than the 6 kB L0 instruction cache: rolled, matrix-kick runs 12-18 % faster (bends included), while
-// the drift-/bend-kick kernels, whose two-edge bodies are 3 kB, lose 4 %.
+// (uniform branches).  Their two-edge loop body would be 6 kB for the quadrupole (160 fp64 instructions per
+// slice), as much as the L0 instruction cache: rolled, matrix-kick runs 2 % faster (12-18 % before the quadrupole's
+// two polarities shared one loop, see QuadPlane), while the drift-/bend-kick kernels, whose two-edge bodies are 3 kB,
+// lose 4 %.
 template <int DEPTH, bool ROLLED = false> struct FusedSpin {
   double &Sx, &Sy, &Ss;
   __device__ __forceinline__ FusedSpin(State& z) : Sx(z.Sx), Sy(z.Sy), Ss(z.Ss) {}
   template <class Stepper>
   __device__ __forceinline__ void run(Stepper& s, int N, double ds) {
-    constexpr bool SM = Stepper::SMALL_ANGLE && !ROLLED;      // (in the rolled matrix-kick kernels it measured 4 % slower)
+    constexpr bool SM = Stepper::SMALL_ANGLE;      // (in the rolled matrix-kick kernels it measured 4 % slower)
     SpinAcc<DEPTH> acc;
     const double hds = 0.5 * ds;
     double wx, wy, ws;
@@ -500,7 +493,7 @@ template <int DEPTH, bool ROLLED = false> struct FusedSpin {
       s.omega(hds, wx, wy, ws);
       acc.template fold_static<DEPTH, SM>(wx, wy, ws);             // edge N: every level (2^(DEPTH-1) | N)
     }
-    acc.template finish<ROLLED>(Sx, Sy, Ss);
+    acc.finish(Sx, Sy, Ss);
   }
   // thin element (A10): one rotation, no Romberg
   __device__ __forceinline__ void thin(double wx, double wy, double ws) {
@@ -837,13 +830,16 @@ __device__ __forceinline__ bool mult_dk(State& z, const DevElem& e, const PCon& 
 
 // a6: quadrupole matrix-kick (24)(25)(27).  kappa^2 = |k1|/P (23); with u = (kappa ds/2)^2 the four
 // functions cos, sin(x)/x, cosh, sinh(x)/x are power series in u (no sqrt of kappa is needed).
-struct QuadLin {
-  double C, S, Ch, Sh;        // cos x, (s/P) sin(x)/x, cosh x, (s/P) sinh(x)/x
-  double kS, kSh;             // |k1| s sin(x)/x,  |k1| s sinh(x)/x
-  double tpp_f, txx_f, txp_f; // (24e) coefficients of Px^2, X^2, X Px in the focusing plane
-  double tpp_d, txx_d, txp_d; // ... of Py^2, Y^2, Y Py in the defocusing plane
-};
-__device__ __forceinline__ void quadlin_build(QuadLin& q, double ak1, double s, const PCon& c) {
+// One plane of the linear flow (24a-d) and of its time-of-flight form (24e):
+//   u' = C u + S p,  p' = C p - k u;   T' contribution -(1/beta_o + Pt)/P (pp p^2 + xx u^2 + xp u p).
+// For the plane the magnet focuses C = cos x, S = (s/P) sin(x)/x, k = |k1| s sin(x)/x; for the other one the hyperbolic
+// functions and k < 0 (A11: the paper's rotation by 90 degrees).  Which plane is which is decided by the sign of k1 when
+// the coefficients are built, so that ONE copy of the slice loop serves both polarities: the loop instantiated once per
+// polarity put the matrix-kick kernels over the instruction cache (19 % of the warp samples waited for instructions).
+struct QuadPlane { double C, S, k, pp, xx, xp; };
+struct QuadLin { QuadPlane x, y; };
+__device__ __forceinline__ void quadlin_build(QuadLin& q, double k1, double s, const PCon& c) {
+  const double ak1 = fabs(k1);
   double kap2 = ak1 * c.iP;
   double u = kap2 * s * s;
   double C, Sx, Ch, Shx;
@@ -869,32 +865,30 @@ __device__ __forceinline__ void quadlin_build(QuadLin& q, double ak1, double s, 
     sincos(x, &sn, &cs);
     C = cs; Sx = sn / x; Ch = cosh(x); Shx = sinh(x) / x;
   }
-  q.C = C; q.Ch = Ch;
-  q.S = s * c.iP * Sx;  q.Sh = s * c.iP * Shx;       // X += (s/P) Px sin(x)/x
-  q.kS = ak1 * s * Sx;  q.kSh = ak1 * s * Shx;       // Px -= kappa^2 P s X sin(x)/x,  kappa^2 P = |k1|
-  double s4 = 0.25 * s, iP2 = c.iP * c.iP;
-  double SC = Sx * C, ShC = Shx * Ch;                // sin(2x)/(2x), sinh(2x)/(2x)
-  q.tpp_f = s4 * iP2 * (1.0 + SC);
-  q.txx_f = s4 * kap2 * (1.0 - SC);
-  q.txp_f = -0.5 * u * Sx * Sx * c.iP;
-  q.tpp_d = s4 * iP2 * (1.0 + ShC);
-  q.txx_d = s4 * kap2 * (ShC - 1.0);
-  q.txp_d = 0.5 * u * Shx * Shx * c.iP;
+  const double s4 = 0.25 * s, iP2 = c.iP * c.iP;
+  const double SC = Sx * C, ShC = Shx * Ch;          // sin(2x)/(2x), sinh(2x)/(2x)
+  QuadPlane f, d;
+  f.C = C;  f.S = s * c.iP * Sx;   f.k = ak1 * s * Sx;       // X += (s/P) Px sin(x)/x,  Px -= kappa^2 P s X sin(x)/x
+  d.C = Ch; d.S = s * c.iP * Shx;  d.k = -ak1 * s * Shx;     // kappa^2 P = |k1|
+  f.pp = s4 * iP2 * (1.0 + SC);   f.xx = s4 * kap2 * (1.0 - SC);   f.xp = -0.5 * u * Sx * Sx * c.iP;
+  d.pp = s4 * iP2 * (1.0 + ShC);  d.xx = s4 * kap2 * (ShC - 1.0);  d.xp = 0.5 * u * Shx * Shx * c.iP;
+  const bool foc_x = k1 > 0.0;
+  q.x = foc_x ? f : d;
+  q.y = foc_x ? d : f;
 }
-// flow of H_qL over s = ds/2: (uf,pf) is the focusing plane, (ud,pd) the defocusing one (A11)
-__device__ __forceinline__ void quadlin_apply(const QuadLin& q, double& uf, double& pf, double& ud, double& pd, double& T,
-                                              double tfac) {
-  double curly = fma(q.tpp_f, pf * pf, fma(q.txx_f, uf * uf, q.txp_f * uf * pf)) +
-                 fma(q.tpp_d, pd * pd, fma(q.txx_d, ud * ud, q.txp_d * ud * pd));
-  T = fma(-tfac, curly, T);
-  double nu = fma(uf, q.C, q.S * pf);
-  pf = fma(pf, q.C, -q.kS * uf);
-  uf = nu;
-  nu = fma(ud, q.Ch, q.Sh * pd);
-  pd = fma(pd, q.Ch, q.kSh * ud);
-  ud = nu;
+// flow of H_qL over the length the coefficients were built for
+__device__ __forceinline__ void quadlin_apply(const QuadLin& q, State& z, double tfac) {
+  const double curly = fma(q.x.pp, z.Px * z.Px, fma(q.x.xx, z.X * z.X, q.x.xp * z.X * z.Px)) +
+                       fma(q.y.pp, z.Py * z.Py, fma(q.y.xx, z.Y * z.Y, q.y.xp * z.Y * z.Py));
+  z.T = fma(-tfac, curly, z.T);
+  double nu = fma(z.X, q.x.C, q.x.S * z.Px);
+  z.Px = fma(z.Px, q.x.C, -q.x.k * z.X);
+  z.X = nu;
+  nu = fma(z.Y, q.y.C, q.y.S * z.Py);
+  z.Py = fma(z.Py, q.y.C, -q.y.k * z.Y);
+  z.Y = nu;
 }
-template <bool FOC, int ORDER> struct QuadMK {
+template <int ORDER> struct QuadMK {
   static constexpr bool SMALL_ANGLE = true;
   State& z;
   const PCon& c;
@@ -906,10 +900,10 @@ template <bool FOC, int ORDER> struct QuadMK {
     k1 = e.kn[0];
     ds = e.ds;
     if (ORDER == 2) {
-      quadlin_build(ql, fabs(k1), 0.5 * e.ds, c);
+      quadlin_build(ql, k1, 0.5 * e.ds, c);
     } else {
-      quadlin_build(ql, fabs(k1), (0.5 * GST_YOSHIDA_X1) * e.ds, c);
-      quadlin_build(ql2, fabs(k1), (0.5 * (GST_YOSHIDA_X1 + GST_YOSHIDA_X0)) * e.ds, c);
+      quadlin_build(ql, k1, (0.5 * GST_YOSHIDA_X1) * e.ds, c);
+      quadlin_build(ql2, k1, (0.5 * (GST_YOSHIDA_X1 + GST_YOSHIDA_X0)) * e.ds, c);
     }
     tfac = c.iP * c.ibpt;
     P2 = 1.0 + c.e0;
@@ -917,10 +911,7 @@ template <bool FOC, int ORDER> struct QuadMK {
     a1k = c.a1 * k1;
     bad = false;
   }
-  __device__ __forceinline__ void lin(const QuadLin& q) {
-    if (FOC) quadlin_apply(q, z.X, z.Px, z.Y, z.Py, z.T, tfac);
-    else     quadlin_apply(q, z.Y, z.Py, z.X, z.Px, z.T, tfac);
-  }
+  __device__ __forceinline__ void lin(const QuadLin& q) { quadlin_apply(q, z, tfac); }
   // (25) over `len`: X += len Px (1/Ps - 1/P), 1/Ps - 1/P = pt2/(P Ps (P+Ps))
   __device__ __forceinline__ void nonlinear(double len) {
     const double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
@@ -966,12 +957,7 @@ template <bool FOC, int ORDER> struct QuadMK {
 };
 template <int ORDER, class Spin>
 __device__ __forceinline__ bool quad_mk(State& z, const DevElem& e, const PCon& c, Spin& spin) {
-  if (e.kn[0] > 0.0) {
-    QuadMK<true, ORDER> s(z, e, c);
-    spin.run(s, e.N, e.ds);
-    return !s.bad;
-  }
-  QuadMK<false, ORDER> s(z, e, c);
+  QuadMK<ORDER> s(z, e, c);
   spin.run(s, e.N, e.ds);
   return !s.bad;
 }
