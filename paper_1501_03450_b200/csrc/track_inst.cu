@@ -1,7 +1,7 @@
 // track_inst.cu -- one translation unit of tracking-kernel instantiations: compiled nine times with
 // -DGST_TU_SPLIT=0|1|2 (drift-, bend-, matrix-kick) and -DGST_TU_GROUP=0|1|2 (see track_launch.cuh).
-// -DGST_ONLY_DEPTH=d (development builds that compile in seconds) keeps the second-order kernels of Romberg depth d
-// alone; every other request fails with cudaErrorNotSupported.
+// -DGST_ONLY_DEPTH=d (development builds that compile in seconds) keeps the kernels of Romberg depth d alone (both
+// orders, no mid-slice orderings); every other request fails with cudaErrorNotSupported.
 #define GST_LAUNCH_IMPL
 #include "track_launch.cuh"
 
@@ -11,7 +11,7 @@
 namespace gst {
 
 #ifdef GST_ONLY_DEPTH
-#define GST_CASE(D, O) case D: if (D != GST_ONLY_DEPTH || O != 2) return cudaErrorNotSupported; else
+#define GST_CASE(D, O) case D: if (D != GST_ONLY_DEPTH) return cudaErrorNotSupported; else
 #else
 #define GST_CASE(D, O) case D:
 #endif
@@ -36,7 +36,9 @@ cudaError_t GST_CAT4(launch_tu, GST_TU_SPLIT, GST_TU_GROUP)(int order, int depth
     GST_CASE(5, 2) return launch_track<S, 5, 2>(rq, st);
     GST_CASE(6, 2) return launch_track<S, 6, 2>(rq, st);
 #endif
-#elif !defined(GST_ONLY_DEPTH)
+#elif defined(GST_ONLY_DEPTH)
+    case GST_ONLY_DEPTH: return launch_track<S, GST_ONLY_DEPTH, 4>(rq, st);
+#else
     case 1: return launch_track<S, 1, 4>(rq, st);
     case 2: return launch_track<S, 2, 4>(rq, st);
     case 3: return launch_track<S, 3, 4>(rq, st);
@@ -68,7 +70,9 @@ cudaError_t GST_CAT4(kernel_info_tu, GST_TU_SPLIT, GST_TU_GROUP)(int order, int 
     GST_CASE(5, 2) return kernel_info<S, 5, 2>(variant, out);
     GST_CASE(6, 2) return kernel_info<S, 6, 2>(variant, out);
 #endif
-#elif !defined(GST_ONLY_DEPTH)
+#elif defined(GST_ONLY_DEPTH)
+    case GST_ONLY_DEPTH: return kernel_info<S, GST_ONLY_DEPTH, 4>(variant, out);
+#else
     case 1: return kernel_info<S, 1, 4>(variant, out);
     case 2: return kernel_info<S, 2, 4>(variant, out);
     case 3: return kernel_info<S, 3, 4>(variant, out);

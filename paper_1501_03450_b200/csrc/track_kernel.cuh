@@ -1211,16 +1211,17 @@ __device__ __forceinline__ bool element_step(int type, State& z, const DevElem& 
 // 85 ms vs 53 ms per 20 turns, profiles/r01_notes.md).
 constexpr int TRACK_BLOCK = 64;
 constexpr int TRACK_MIN_BLOCKS = 8;
-// The fourth-order matrix-kick map carries two tables of linear-flow coefficients: at 128 registers it spills
-// 800 B per thread.  With 6 blocks per SM (3 warps per sub-partition, 167 registers, no spills) it measured 20 %
-// faster; every other instantiation is equal or slightly slower that way (profiles/r01_notes.md).
+// The fourth-order matrix-kick and drift-kick maps (two coefficient tables; three kicks and four curved drifts per
+// slice) spill 800 B per thread at 128 registers.  With 6 blocks per SM (3 warps per sub-partition, 168 registers) they
+// measured 20 % and 5 % faster; fourth-order bend-kick is 3 % slower that way and stays at 8, like every second-order
+// kernel.
 // A bunch of at most two warps per sub-partition is not short of registers but of parallelism: one warp's dependency
 // chains set the time.  The FAT variant is compiled for 4 blocks per SM (up to 255 registers; ptxas takes 170-190, no
 // spills, more of the loop bodies in flight): measured +7 % (bend-kick) to +18 % (matrix-kick, with its two-edge loop
 // bodies) on 4096-particle bunches, +7 % at 16 384.
 constexpr int TRACK_FAT_BLOCKS = 4;
 __host__ __device__ constexpr int track_min_blocks(int split, int order, bool fat) {
-  return fat ? TRACK_FAT_BLOCKS : (split == SPLIT_MK && order == 4) ? 6 : TRACK_MIN_BLOCKS;
+  return fat ? TRACK_FAT_BLOCKS : (order == 4 && split != SPLIT_BK) ? 6 : TRACK_MIN_BLOCKS;
 }
 
 // a0: the lattice is ALWAYS read from shared memory (LDS; element records and sequence entries through a pointer that
