@@ -888,13 +888,32 @@ __device__ __forceinline__ void quadlin_apply(const QuadLin& q, State& z, double
   z.Py = fma(z.Py, q.y.C, -q.y.k * z.Y);
   z.Y = nu;
 }
+// 1/Ps for a particle of total momentum P and transverse momentum pt: with eps = pt^2/P^2,
+//   1/Ps = (1/P)(1 - eps)^(-1/2) = (1/P)[1 + eps h(eps)],  h = 1/2 + 3/8 eps + 5/16 eps^2 + 35/128 eps^3 + ...
+// In a quadrupole P is a constant of the element, so the kick of H_qNL (25) and the 1/Ps of Omega need neither a
+// reciprocal square root nor a reciprocal while eps <= 2^-13 (angles up to 11 mrad; the truncation error of h is then
+// 63/256 eps^4 = 5e-17, half an ulp): (25a) uses 1/Ps - 1/P = eps h/P, (25e)'s bracket 1/Ps - 1/P - pt^2/(2P^3) =
+// eps^2 (3/8 + 5/16 eps + 35/128 eps^2)/P.  Larger angles take the exact forms, out of line.
+#define GST_MK_EPS_MAX 1.220703125e-4   // 2^-13
+struct QuadNL { double d, br, iPs; bool ok; };   // 1/Ps - 1/P, the bracket of (25e), 1/Ps
+static __device__ __noinline__ QuadNL quadnl_exact(double pt2, double P, double iP) {
+  QuadNL r;
+  const double ps2 = fma(P, P, -pt2);
+  r.ok = is_pos(ps2);
+  r.iPs = rsqrt_nr(ps2);
+  const double Ps = ps2 * r.iPs;
+  const double t = r.iPs * rcp_nr(P + Ps);           // 1/(Ps (P+Ps))
+  r.d = pt2 * iP * t;                                // 1/Ps - 1/P = pt2/(P Ps (P+Ps))
+  r.br = pt2 * pt2 * fma(2.0, P, Ps) * (0.5 * iP * iP * iP) * t * (t * Ps);   // pt2^2 (2P+Ps)/(2 P^3 Ps (P+Ps)^2)
+  return r;
+}
 template <int ORDER> struct QuadMK {
   static constexpr bool SMALL_ANGLE = true;
   State& z;
   const PCon& c;
   QuadLin ql;       // linear flow over ds/2 (second order) or x1 ds/2 (fourth order)
   QuadLin ql2;      // fourth order only: linear flow over (x1 + x0) ds/2 < 0
-  double k1, ds, tfac, P2, hiP3, a1k;
+  double k1, ds, tfac, iP2, a1k;
   bool bad;
   __device__ __forceinline__ QuadMK(State& z_, const DevElem& e, const PCon& c_) : z(z_), c(c_) {
     k1 = e.kn[0];
@@ -906,25 +925,26 @@ template <int ORDER> struct QuadMK {
       quadlin_build(ql2, k1, (0.5 * (GST_YOSHIDA_X1 + GST_YOSHIDA_X0)) * e.ds, c);
     }
     tfac = c.iP * c.ibpt;
-    P2 = 1.0 + c.e0;
-    hiP3 = 0.5 * c.iP * c.iP * c.iP;
+    iP2 = c.iP * c.iP;
     a1k = c.a1 * k1;
     bad = false;
   }
   __device__ __forceinline__ void lin(const QuadLin& q) { quadlin_apply(q, z, tfac); }
-  // (25) over `len`: X += len Px (1/Ps - 1/P), 1/Ps - 1/P = pt2/(P Ps (P+Ps))
+  // (25) over `len`: X += len Px (1/Ps - 1/P);  T' = -(1/beta0+Pt)[1/Ps - 1/P - pt2/(2P^3)] + tq
   __device__ __forceinline__ void nonlinear(double len) {
     const double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
-    const double ps2 = P2 - pt2;
-    bad |= !is_pos(ps2);
-    const double iPs = rsqrt_nr(ps2);
-    const double Ps = ps2 * iPs;
-    const double t = iPs * rcp_nr(c.P + Ps);         // 1/(Ps (P+Ps))
-    const double d = pt2 * c.iP * t;
+    const double eps = pt2 * iP2;
+    const double ie = c.iP * eps;
+    const double h2 = fma(fma(35.0 / 128.0, eps, 5.0 / 16.0), eps, 3.0 / 8.0);
+    double d = ie * fma(h2, eps, 0.5);
+    double br = ie * eps * h2;
+    if (__builtin_expect(!(eps <= GST_MK_EPS_MAX), 0)) {
+      const QuadNL x = quadnl_exact(pt2, c.P, c.iP);
+      d = x.d; br = x.br;
+      bad |= !x.ok;
+    }
     z.X = fma(len * d, z.Px, z.X);
     z.Y = fma(len * d, z.Py, z.Y);
-    // T' = -(1/beta0+Pt)[1/Ps - 1/P - pt2/(2P^3)] + tq,  bracket = pt2^2 (2P+Ps)/(2 P^3 Ps (P+Ps)^2)
-    const double br = pt2 * pt2 * fma(2.0, c.P, Ps) * hiP3 * t * (t * Ps);
     z.T = fma(len, fma(-c.ibpt, br, c.tq), z.T);
   }
   __device__ __forceinline__ void advance() {
@@ -945,9 +965,14 @@ template <int ORDER> struct QuadMK {
   template <bool DKSKD> __device__ __forceinline__ void pwc_first() { advance(); }     // not a drift-kick map: half slice
   template <bool DKSKD> __device__ __forceinline__ void pwc_second() { advance(); }
   __device__ __forceinline__ void omega(double w, double& wx, double& wy, double& ws) {
-    const double ps2 = P2 - fma(z.Px, z.Px, z.Py * z.Py);
-    bad |= !is_pos(ps2);
-    const double iPs = rsqrt_nr(ps2);
+    const double pt2 = fma(z.Px, z.Px, z.Py * z.Py);
+    const double eps = pt2 * iP2;
+    double iPs = fma(c.iP * eps, fma(fma(fma(35.0 / 128.0, eps, 5.0 / 16.0), eps, 3.0 / 8.0), eps, 0.5), c.iP);
+    if (__builtin_expect(!(eps <= GST_MK_EPS_MAX), 0)) {
+      const QuadNL x = quadnl_exact(pt2, c.P, c.iP);
+      iPs = x.iPs;
+      bad |= !x.ok;
+    }
     const double pb = c.a2p * k1 * (z.Px * z.Y + z.Py * z.X);
     const double wi = -w * iPs;
     wx = wi * fma(a1k, z.Y, -pb * z.Px);

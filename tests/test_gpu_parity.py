@@ -231,6 +231,27 @@ def test_rectangular_bends_in_a_ring(gst, O, depth, n_slices):
     assert abs(g_gpu - g_ref) < 1e-12 * g_ref                 # the cavity sees the same circumference (arc lengths)
 
 
+@pytest.mark.parametrize("split", [W.SPLIT_MATRIX_KICK, W.SPLIT_MATRIX_KICK_4])
+def test_matrix_kick_at_large_transverse_momenta(gst, O, split):
+    """The matrix-kick quadrupole takes 1/Ps from a series in pt^2/P^2 up to 2^-13 (angles of 11 mrad) and from the
+    exact forms beyond (csrc/track_kernel.cuh: QuadMK): a bunch with angles from 0 to 47 mrad exercises both, in one
+    warp, in the small-bunch and in the occupancy-oriented build of the kernel."""
+    lat = W.lattice([W.drift(0.3), W.quad(0.5, +0.8), W.drift(0.2), W.quad(0.5, -0.8), W.drift(0.3)] * 2)
+    bm = W.beam(5.0)
+    st = W.gaussian_bunch(3, 200, 5.0, 2e-3, 2e-2, 2e-3, 2e-2, 1e-3, 0.01, "sphere")
+    st[1, :40] *= 0.01                                   # some particles well inside the series' range
+    st[3, :40] *= 0.01
+    eps = (st[1] ** 2 + st[3] ** 2)
+    assert (eps < 1e-5).sum() >= 30 and (eps > 2e-4).sum() >= 100
+    ref, rlost, _ = O.track(lat, bm, st, 1, split, 8, 4)
+    assert not rlost.any()
+    for lean in (False, True):
+        got, lost, *_ = gpu_track(gst, lat, bm, st, 1, split, 8, 4, lean=lean)
+        assert not lost.any()
+        assert orbit_err(got, ref) < 1e-12 and orbit_err_per_particle(got, ref) < 1e-12, (lean, orbit_err_per_particle(got, ref))
+        assert spin_err(got, ref) < 1e-12, (lean, spin_err(got, ref))
+
+
 def test_large_angle_per_slice_takes_the_sincos_branch(gst, O):
     # one slice through a strong bend at high G*gamma: rotation angle per edge > 1.4 rad
     lat = W.lattice([W.sbend(9.45, 0.2), W.drift(1.0)])
