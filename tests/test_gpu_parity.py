@@ -491,6 +491,42 @@ def test_random_lattices_of_every_element_type(gst, O, seed):
     assert abs(g_gpu - g_ref) < 1e-12 * g_ref
 
 
+@pytest.mark.parametrize("case", ["only_drifts", "only_markers", "trailing_drifts", "drift_before_every_type", "leading_and_split_drifts"])
+def test_lattice_compiler_edge_cases(gst, O, case):
+    """gst_lattice_create merges runs of drifts into the element behind them and drops markers (csrc/gst_api.cu); the
+    oracle goes through the user's lattice element by element.  The edges: rings of drifts or markers only, drifts left
+    at the end of the ring (a hard boundary: no wrap-around into the first element), a drift space in front of EVERY
+    element type, drifts cut into pieces with markers between them."""
+    ang = 2 * math.pi / 40
+    if case == "only_drifts":
+        els = [W.drift(0.5), W.drift(1.25), W.marker(), W.drift(0.25)]
+    elif case == "only_markers":
+        els = [W.marker(), W.marker()]
+    elif case == "trailing_drifts":
+        els = [W.quad(0.4, 0.5), W.drift(0.3), W.sbend(1.0, ang), W.drift(0.7), W.marker(), W.drift(0.2)]
+    elif case == "drift_before_every_type":
+        els = []
+        for e in (W.quad(0.4, 0.5), W.quad(0.4, -0.5), W.sbend(1.0, ang), W.multipole(0.3, kn=(0.02, 0.9, -4.0, 30.0)),
+                  W.thin_sextupole(0.4), W.cavity(1e5, 3.0, 0.1, +1.0), W.snake(2.0, 0.3), W.fringe(+1.0, 0.02, (0.3, 0, 0, 0)),
+                  W.solenoid(0.8, 0.2), W.rbend(1.2, 0.05), W.marker()):
+            els += [W.drift(0.37), e]
+    else:
+        els = [W.drift(0.2), W.marker(), W.drift(0.3), W.drift(0.1), W.quad(0.4, 0.5), W.drift(0.6), W.marker(), W.drift(0.4),
+               W.sbend(1.0, ang), W.marker(), W.thin_sextupole(-0.3), W.drift(0.5)]
+    lat = W.lattice(els)
+    bm = W.beam(8.0)
+    st = W.gaussian_bunch(61, 100, 8.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
+    L = gst.Lattice(lat, bm)
+    assert L.steps_per_turn(4) == W.steps_per_turn(lat, 4)          # the metric counts the USER lattice
+    L.close()
+    for split in (W.SPLIT_DRIFT_KICK, W.SPLIT_BEND_KICK, W.SPLIT_MATRIX_KICK):
+        ref, rlost, g_ref = O.track(lat, bm, st, 3, split, 4, 3)
+        got, lost, pol, emit, g_gpu = gpu_track(gst, lat, bm, st, 3, split, 4, 3)
+        assert not rlost.any() and not lost.any()
+        assert orbit_err(got, ref) < 2e-12 and spin_err(got, ref) < 2e-12, (split, orbit_err(got, ref), spin_err(got, ref))
+        assert abs(g_gpu - g_ref) < 1e-12 * g_ref
+
+
 def test_lattice_with_hundreds_of_unique_elements(gst, O):
     """A ring whose magnets all differ slightly (as a real machine's do): 448 unique records = 287 kB of element
     table, read from global memory instead of shared memory; the sequence alone still fits."""
