@@ -211,6 +211,24 @@ gst_status gst_bunch_set_reference(gst_bunch* b, const gst_beam* beam, int64_t t
 gst_status gst_track_host(const gst_lattice* lat, double* const host_state[9], size_t n, int64_t n_turns,
                           gst_split split, int n_slices, int romberg_depth, double out_pol[4], int64_t* out_lost);
 
+/* Bunch polarization WITHOUT ANY ALLOCATION, for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it) and so cannot make a gst_bunch.  The same two-stage reduction as
+ * gst_polarization, with its per-block partial sums in a fixed device array inside the library (128 KiB that every
+ * GPU which loads the library holds until the process exits) instead of memory from gst_bunch_init.
+ *   sx, sy, ss  DEVICE arrays of n doubles: the spin components (borrowed, read only)
+ *   lost        DEVICE array of n bytes, non-zero = excluded (A15/A18), or NULL: nobody is lost
+ *   n           particles; at most GST_NOALLOC_MAX_PARTICLES, else GST_EINVAL (the scratch array is what it is)
+ *   out_dev     DEVICE array of 5 doubles: {Px, Py, Ps, |P|, number of particles counted}
+ * ASYNCHRONOUS on `cuda_stream`: two kernels are enqueued, nothing is synchronised, nothing is copied to the host.
+ * Calls no cudaMalloc, cudaFree or allocating library routine.  Runs on the device that owns out_dev; the inputs must
+ * live there.  Every call on a device shares the one scratch array, which keeps the last call's contents (none of it
+ * has to start at zero: a call overwrites every record it later reads): calls that OVERLAP on the GPU -- different
+ * streams without an event between them, several host threads -- race on it and give wrong sums; calls on one stream
+ * are safe.  (The first call on a device asks the driver for the array's address: make it before a capture begins.)  */
+#define GST_NOALLOC_MAX_PARTICLES 1048576
+gst_status gst_polarization_noalloc(const double* sx, const double* sy, const double* ss, const uint8_t* lost, size_t n,
+                                    double* out_dev, void* cuda_stream);
+
 /* Thread-local message for the last error on this thread; never NULL. */
 const char* gst_last_error(void);
 

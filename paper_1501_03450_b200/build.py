@@ -2,7 +2,7 @@
 
 The kernel instantiations are spread over nine translation units (csrc/track_inst.cu compiled with different
 -DGST_TU_SPLIT / -DGST_TU_GROUP) so that the nvcc runs go in parallel on every host core; objects are kept under
-csrc/build/ (git-ignored)."""
+csrc/build/ (git-ignored) and recompiled only when something their unit includes has changed."""
 import os
 import subprocess
 import sys
@@ -10,15 +10,26 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
-# (object name, source, extra defines): the API, the diagnostics and nine units of kernel instantiations
-UNITS = [("gst_api", "gst_api.cu", []), ("gst_diag", "gst_diag.cu", [])] + \
-    [("track_inst_s%dg%d" % (sp, g), "track_inst.cu", ["-DGST_TU_SPLIT=%d" % sp, "-DGST_TU_GROUP=%d" % g])
+INC = os.path.join(os.path.dirname(HERE), "include")
+TRACK_HEADERS = ["track_kernel.cuh", "track_chain_kernel.cuh", "track_launch.cuh"]
+# (object name, source, extra defines, headers it includes): the API, the diagnostics, the allocation-free entry point
+# and nine units of kernel instantiations
+UNITS = [("gst_api", "gst_api.cu", [], TRACK_HEADERS + ["reduce_kernel.cuh", "gst_internal.h", "gst.h", "gst_diag.h"]),
+         ("gst_diag", "gst_diag.cu", [], TRACK_HEADERS + ["gst_internal.h", "gst.h", "gst_diag.h"]),
+         ("gst_noalloc", "gst_noalloc.cu", [], ["gst_internal.h", "gst.h"])] + \
+    [("track_inst_s%dg%d" % (sp, g), "track_inst.cu", ["-DGST_TU_SPLIT=%d" % sp, "-DGST_TU_GROUP=%d" % g], TRACK_HEADERS)
      for g in (1, 2, 0) for sp in (2, 1, 0)]            # the slowest units first
-DEPS = [os.path.join(CSRC, f) for f in ("gst_api.cu", "gst_diag.cu", "track_inst.cu", "track_kernel.cuh",
-                                        "track_chain_kernel.cuh", "track_launch.cuh", "reduce_kernel.cuh",
-                                        "gst_internal.h")] + \
-    [os.path.join(os.path.dirname(HERE), "include", f) for f in ("gst.h", "gst_diag.h")] + \
-    [os.path.abspath(__file__)]   # the flags live in this file
+
+
+def _path(f):
+    return os.path.join(INC if f in ("gst.h", "gst_diag.h") else CSRC, f)
+
+
+def _unit_deps(src, headers):
+    return [_path(src)] + [_path(h) for h in headers] + [os.path.abspath(__file__)]   # the flags live in this file
+
+
+DEPS = sorted({d for _, src, _, hdrs in UNITS for d in _unit_deps(src, hdrs)})
 OUT = os.path.join(HERE, "libgst.so")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC"]
@@ -43,11 +54,18 @@ def build(force: bool = False, verbose: bool = False) -> str:
         return OUT
     nvcc = os.environ.get("NVCC", "nvcc")
     os.makedirs(OBJ, exist_ok=True)
-    objs, pending, running = [], list(UNITS), []
+    objs, pending, running = [], [], []
+    for unit in UNITS:          # an object is kept when it is newer than everything its unit is compiled from
+        obj = os.path.join(OBJ, unit[0] + ".o")
+        fresh = os.path.exists(obj) and os.path.getmtime(obj) >= max(os.path.getmtime(d) for d in _unit_deps(unit[1], unit[3]))
+        if fresh and not force and not verbose:
+            objs.append(obj)
+        else:
+            pending.append(unit)
     workers = max(1, min(len(UNITS), os.cpu_count() or 1))
     while pending or running:
         while pending and len(running) < workers:
-            name, src, defs = pending.pop(0)
+            name, src, defs, _ = pending.pop(0)
             obj = os.path.join(OBJ, name + ".o")
             if name == "gst_diag":
                 defs = defs + ['-DGST_KERNEL_SOURCE_HASH="%s"' % kernel_source_hash()]

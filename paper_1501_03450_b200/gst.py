@@ -39,7 +39,9 @@ _dp = C.POINTER(C.c_double)
 EXPORTS = ["gst_lattice_create", "gst_lattice_destroy", "gst_lattice_steps_per_turn", "gst_bunch_init",
            "gst_bunch_destroy", "gst_track", "gst_polarization", "gst_emittance", "gst_bunch_lost",
            "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host", "gst_last_error",
-           "gst_bunch_set_launch", "gst_bunch_status", "gst_track_pwc", "gst_bunch_last_kernel"]
+           "gst_bunch_set_launch", "gst_bunch_status", "gst_track_pwc", "gst_bunch_last_kernel",
+           "gst_polarization_noalloc"]
+NOALLOC_MAX_PARTICLES = 1 << 20
 LAUNCH_AUTO, LAUNCH_STATIC, LAUNCH_LEAN = 0, 1, 2
 
 
@@ -73,6 +75,8 @@ def lib():
         L.gst_bunch_set_reference.argtypes = [vp, C.POINTER(gst_beam), C.c_int64]
         L.gst_track_host.argtypes = [vp, C.POINTER(_dp), C.c_size_t, C.c_int64, C.c_int, C.c_int, C.c_int, _dp,
                                      C.POINTER(C.c_int64)]
+        L.gst_polarization_noalloc.argtypes = [vp, vp, vp, vp, C.c_size_t, vp, vp]
+        L.gst_polarization_noalloc.restype = C.c_int
         L.gst_bunch_set_launch.argtypes = [vp, C.c_int]
         L.gst_bunch_status.argtypes = [vp, vp]
         for name in ("gst_lattice_create", "gst_bunch_init", "gst_track", "gst_polarization", "gst_emittance",
@@ -230,3 +234,20 @@ class Bunch:
             self.close()
         except Exception:
             pass
+
+
+def polarization_noalloc(sx, sy, ss, lost, out, stream=None):
+    """gst_polarization_noalloc: sx, sy, ss float64 CUDA tensors of n elements, lost a uint8 CUDA tensor or None, out a
+    float64 CUDA tensor of 5 elements that receives {Px, Py, Ps, |P|, counted}.  Asynchronous; allocates nothing."""
+    import torch
+    n = sx.numel()
+    for t in (sx, sy, ss):
+        assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == n
+    assert out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() >= 5
+    lp = None
+    if lost is not None:
+        assert lost.is_cuda and lost.dtype == torch.uint8 and lost.is_contiguous() and lost.numel() == n
+        lp = C.c_void_p(lost.data_ptr())
+    s = torch.cuda.current_stream() if stream is None else stream
+    _check(lib().gst_polarization_noalloc(C.c_void_p(sx.data_ptr()), C.c_void_p(sy.data_ptr()), C.c_void_p(ss.data_ptr()),
+                                          lp, n, C.c_void_p(out.data_ptr()), C.c_void_p(s.cuda_stream)))
