@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "build")
 INC = os.path.join(os.path.dirname(HERE), "include")
-TRACK_HEADERS = ["track_kernel.cuh", "track_chain_kernel.cuh", "track_launch.cuh"]
+TRACK_HEADERS = ["track_kernel.cuh", "track_chain_kernel.cuh", "track_split_kernel.cuh", "track_launch.cuh"]
 # (object name, source, extra defines, headers it includes): the API, the diagnostics, the allocation-free entry point
 # and nine units of kernel instantiations
 UNITS = [("gst_api", "gst_api.cu", [], TRACK_HEADERS + ["reduce_kernel.cuh", "gst_internal.h", "gst.h", "gst_diag.h"]),
@@ -35,7 +35,7 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "-Xcompiler", "-fPIC"]
 
 
-KERNEL_SOURCES = ("track_kernel.cuh", "track_chain_kernel.cuh", "track_launch.cuh", "track_inst.cu")
+KERNEL_SOURCES = ("track_kernel.cuh", "track_chain_kernel.cuh", "track_split_kernel.cuh", "track_launch.cuh", "track_inst.cu")
 
 
 def kernel_source_hash() -> str:

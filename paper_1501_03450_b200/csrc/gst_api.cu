@@ -522,6 +522,7 @@ static gst_status track_impl(gst_bunch* b, const gst_lattice* lat, int64_t n_tur
   rq.sms = lat->sms;
   rq.allow_chain = b->launch_mode == GST_LAUNCH_AUTO;
   rq.allow_fat = b->launch_mode != GST_LAUNCH_LEAN;
+  rq.allow_split = b->launch_mode == GST_LAUNCH_AUTO;
   rq.chain.scratch = b->d_chain;
   rq.chain.flag = b->d_chain + gst::CHAIN_SCRATCH_INTS;
   rq.chain.E0 = b->d_chain_E0;

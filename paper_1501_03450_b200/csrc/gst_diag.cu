@@ -143,8 +143,9 @@ gst_status gst_diag_kernel_info(gst_split split, int romberg_depth, int variant,
                                 int* out_max_blocks_per_sm) {
   if ((int)split < 0 || (int)split > 5 || romberg_depth < 1 || romberg_depth > 6) return fail(GST_EINVAL, "unknown split or depth");
   const int order = (int)split >= 3 ? 4 : 2;
-  if (variant < 0 || variant > 2) return fail(GST_EINVAL, "unknown kernel variant %d", variant);
-  if (variant == 1 && order == 4) return fail(GST_EINVAL, "the rotating launch exists for the second-order splits only");
+  if (variant < 0 || variant > 3) return fail(GST_EINVAL, "unknown kernel variant %d", variant);
+  if ((variant == 1 || variant == 3) && order == 4)
+    return fail(GST_EINVAL, "the rotating launch and the two-warp kernel exist for the second-order splits only");
   gst::KernelInfo ki;
   const cudaError_t ce = gst::kernel_info_of((int)split % 3, order, romberg_depth, variant, &ki);
   if (ce != cudaSuccess) return fail(GST_ECUDA, "kernel attributes: %s", cudaGetErrorString(ce));

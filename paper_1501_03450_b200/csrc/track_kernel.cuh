@@ -1161,7 +1161,7 @@ static __constant__ double FRINGE_INV_M[4] = {1.0 / 2.0, 1.0 / 3.0, 1.0 / 4.0, 1
 // the element types that take a merged drift space in front of them the plain way (see element_step)
 template <int SPLIT, int ORDER, class Spin>
 __device__ __forceinline__ bool element_step_other(int type, State& z, const DevElem& e, PCon& pc, Ref& ref, double G, Spin& spin) {
-  if (type == K_QUAD) return quad_mk<ORDER>(z, e, pc, spin);
+  if (SPLIT == SPLIT_MK && type == K_QUAD) return quad_mk<ORDER>(z, e, pc, spin);   // the other splits never get here with a quadrupole
   if (type == K_THIN) {   // A10: half kick, spin, half kick
     double bx, by, wx, wy, ws;
     mult_field(e, z.X, z.Y, bx, by);

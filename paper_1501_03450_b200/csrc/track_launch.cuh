@@ -8,6 +8,7 @@
 
 #include "track_chain_kernel.cuh"
 #include "track_kernel.cuh"
+#include "track_split_kernel.cuh"
 
 namespace gst {
 
@@ -19,6 +20,7 @@ struct LaunchRequest {
   int sms = 0;                  // SMs of the bunch's device
   bool allow_chain = false;     // GST_LAUNCH_AUTO: the planner may take the rotating launch
   bool allow_fat = true;        // not GST_LAUNCH_LEAN: small bunches take the variant with registers to spare
+  bool allow_split = false;     // GST_LAUNCH_AUTO: the smallest bunches take the kernel with orbit and spin in two warps
   ChainArgs chain;              // the bunch's scratch for it (n_chains, chunk_turns, poll_limit are filled in here)
   long long poll_limit_override = 0;   // != 0: fault injection (include/gst_diag.h)
   const char* kernel = "";      // out: name of the kernel launched
@@ -57,7 +59,7 @@ inline int tu_group(int order, int depth) { return order == 4 ? 2 : (depth >= 4 
 inline cudaError_t launch_tracking(int split3, int order, int depth, LaunchRequest& rq, cudaStream_t st) {
   GST_DISPATCH_TU(launch_tu, order, depth, rq, st)
 }
-// variant: 0 = track_kernel, 1 = track_chain_kernel, 2 = track_kernel (FAT)
+// variant: 0 = track_kernel, 1 = track_chain_kernel, 2 = track_kernel (FAT), 3 = track_split_kernel
 inline cudaError_t kernel_info_of(int split3, int order, int depth, int variant, KernelInfo* out) {
   GST_DISPATCH_TU(kernel_info_tu, order, depth, variant, out)
 }
@@ -108,6 +110,13 @@ inline bool chain_plan(long long n, long long n_turns, long long steps_per_turn,
   return true;
 }
 
+// Bunches that take the two-warp kernel: its 2 x ceil(n / 32) warps each find a sub-partition of their own.
+// GST_SPLIT_MAX_WARPS_PER_SM (a build-time override for measurements) counts particle warps per SM.
+#ifndef GST_SPLIT_MAX_WARPS_PER_SM
+#define GST_SPLIT_MAX_WARPS_PER_SM 4
+#endif
+inline long long split_max_warps(int sms) { return (long long)GST_SPLIT_MAX_WARPS_PER_SM * sms; }
+
 template <int SPLIT, int DEPTH, int ORDER>
 cudaError_t launch_track(LaunchRequest& rq, cudaStream_t st) {
   TrackArgs& a = rq.args;
@@ -138,6 +147,19 @@ cudaError_t launch_track(LaunchRequest& rq, cudaStream_t st) {
       }
     }
   }
+  if constexpr (ORDER == 2 && DEPTH >= 1) {
+    // T1s: at most one warp of particles per two sub-partitions -- orbit and spin of a particle in two warps, each
+    // with a sub-partition (and its FP64 pipe) to itself (track_split_kernel.cuh)
+    if (rq.allow_split && !p.streamed && (a.n + 31) / 32 <= split_max_warps(rq.sms)) {
+      auto sk = track_split_kernel<SPLIT, DEPTH>;
+      const size_t bytes = split_ring_offset(a.n_unique, a.n_seq) + SPLIT_RING_BYTES;
+      cudaError_t e = cudaFuncSetAttribute(sk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+      if (e != cudaSuccess) return e;
+      sk<<<(unsigned)((a.n + 31) / 32), SPLIT_BLOCK, bytes, st>>>(a);
+      rq.kernel = "track_split_kernel";
+      return cudaGetLastError();
+    }
+  }
   // T1: one thread per particle; shared memory kept small so that 8 blocks of 64 threads stay resident
   // at most two warps per sub-partition: the variant with registers to spare (track_kernel.cuh: FAT)
   const bool fat = rq.allow_fat && !p.streamed && (a.n + 31) / 32 <= 2LL * 4 * rq.sms;
@@ -154,15 +176,17 @@ template <int SPLIT, int DEPTH, int ORDER>
 cudaError_t kernel_info(int variant, KernelInfo* out) {
   const void* f = variant == 2 ? (const void*)track_kernel<SPLIT, DEPTH, ORDER, false, true>
                                : (const void*)track_kernel<SPLIT, DEPTH, ORDER, false, false>;
+  int block = TRACK_BLOCK;
   if constexpr (ORDER == 2 && DEPTH >= 1) {
     if (variant == 1) f = (const void*)track_chain_kernel<SPLIT, DEPTH, ORDER>;
+    if (variant == 3) { f = (const void*)track_split_kernel<SPLIT, DEPTH>; block = SPLIT_BLOCK; }
   }
   cudaFuncAttributes at;
   cudaError_t e = cudaFuncGetAttributes(&at, f);
   if (e != cudaSuccess) return e;
   out->registers = at.numRegs;
   out->local_bytes = (int)at.localSizeBytes;
-  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&out->blocks_per_sm, f, TRACK_BLOCK, 0);
+  return cudaOccupancyMaxActiveBlocksPerMultiprocessor(&out->blocks_per_sm, f, block, 0);
 }
 }  // namespace
 #endif  // GST_LAUNCH_IMPL

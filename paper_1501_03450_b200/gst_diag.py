@@ -62,7 +62,7 @@ def kernel_source_hash():
     return lib().gst_diag_kernel_source_hash().decode()
 
 
-KERNEL_VARIANTS = {"track_kernel": 0, "track_chain_kernel": 1, "track_kernel_fat": 2}
+KERNEL_VARIANTS = {"track_kernel": 0, "track_chain_kernel": 1, "track_kernel_fat": 2, "track_split_kernel": 3}
 
 
 def kernel_info(split, depth, kernel="track_kernel"):

@@ -126,17 +126,21 @@ def test_all_splits_depths_all_element_types(gst, O, split, depth, n_slices):
     n = 200                                   # 3 full blocks of 64 and a ragged tail of 8
     st = W.gaussian_bunch(7, n, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
     ref, rlost, g_ref = O.track(lat, bm, st, 2, split, n_slices, depth)
-    # 200 particles take the small-bunch kernel variant; the variant large bunches get must give the same
-    got, lost, pol, emit, g_gpu = gpu_track(gst, lat, bm, st, 2, split, n_slices, depth, want_kernel="track_kernel_fat")
+    # 200 particles take a small-bunch kernel: orbit and spin in two warps for the second-order splits, else the fused
+    # kernel with registers to spare; the fused variants (the one large bunches get included) must give the same
+    auto = "track_split_kernel" if split < 3 else "track_kernel_fat"
+    got, lost, pol, emit, g_gpu = gpu_track(gst, lat, bm, st, 2, split, n_slices, depth, want_kernel=auto)
+    fat = gpu_track(gst, lat, bm, st, 2, split, n_slices, depth, static=True, want_kernel="track_kernel_fat")
     lean = gpu_track(gst, lat, bm, st, 2, split, n_slices, depth, lean=True, want_kernel="track_kernel")
     assert not rlost.any() and not lost.any()
     assert orbit_err(got, ref) < 2e-12, orbit_err(got, ref)
     assert spin_err(got, ref) < 2e-12, spin_err(got, ref)
     assert abs(g_gpu - g_ref) < 1e-12 * g_ref
     assert np.max(np.abs(np.linalg.norm(got[6:9], axis=0) - 1)) < 1e-12     # A9: |S| = 1 without renormalising
-    assert orbit_err(lean[0], ref) < 2e-12 and spin_err(lean[0], ref) < 2e-12 and lean[4] == g_gpu
-    # the same source compiled twice: the two differ by the compiler's choice of fused multiply-adds only
-    assert orbit_err(lean[0], got) < 1e-13 and spin_err(lean[0], got) < 1e-13
+    for other in (fat, lean):
+        assert orbit_err(other[0], ref) < 2e-12 and spin_err(other[0], ref) < 2e-12 and other[4] == g_gpu
+        # the same source compiled again: the kernels differ by the compiler's choice of fused multiply-adds only
+        assert orbit_err(other[0], got) < 1e-13 and spin_err(other[0], got) < 1e-13
 
 
 @pytest.mark.parametrize("split", [W.SPLIT_DRIFT_KICK_4, W.SPLIT_BEND_KICK_4, W.SPLIT_MATRIX_KICK_4])
@@ -372,6 +376,38 @@ def test_chain_rotation_every_split_and_low_depths(gst, split, depth, n_slices):
     keep = ~sta[1].astype(bool)
     assert np.array_equal(rot[0][:, keep], sta[0][:, keep])
     assert np.array_equal(rot[2], sta[2]) and rot[4] == sta[4]
+
+
+@pytest.mark.parametrize("split", [W.SPLIT_DRIFT_KICK, W.SPLIT_BEND_KICK, W.SPLIT_MATRIX_KICK])
+@pytest.mark.parametrize("depth,n_slices", [(1, 1), (1, 3), (2, 2), (3, 4), (4, 8), (5, 16), (6, 32)])
+def test_two_warp_kernel_agrees_with_the_fused_kernel(gst, O, split, depth, n_slices):
+    """Small bunches take the kernel that gives a particle's orbit and its spin to two warps
+    (csrc/track_split_kernel.cuh): the same functions as the fused kernel, compiled a second time, so the two agree to
+    rounding; lost flags and the ramping reference energy exactly.  Every element type, a ragged last block, lost
+    particles in the first and in the last block, enough turns for the ring of rotation vectors to wrap many times;
+    and the two-warp kernel against the oracle."""
+    ang = 2 * math.pi / 24
+    fr = ((0.3, 2.0, 0.0, 0.0), (0.1, 0.0, 0.0, 0.0))
+    lat = np.concatenate([mixed_lattice(ramp=True), W.lattice([
+        W.solenoid(0.8, 0.12), W.drift(0.3), W.rbend(1.5, ang / 2), W.fringe(+1.0, 0.02, *fr), W.quad(0.5, 0.2),
+        W.fringe(-1.0, 0.02, *fr), W.marker(), W.drift(0.2)])])
+    bm = W.beam(12.0)
+    n = 3 * 32 + 5
+    st = W.gaussian_bunch(41, n, 12.0, 2e-3, 3e-4, 2e-3, 3e-4, 5e-4, 0.05, "sphere")
+    st[1, 3] = 1.5
+    st[3, n - 2] = -2.0
+    turns = 3
+    two = gpu_track(gst, lat, bm, st, turns, split, n_slices, depth, want_kernel="track_split_kernel")
+    one = gpu_track(gst, lat, bm, st, turns, split, n_slices, depth, static=True, want_kernel="track_kernel_fat")
+    assert np.array_equal(two[1], one[1]) and two[1][3] and two[1][n - 2] and two[1].sum() == 2
+    keep = ~one[1].astype(bool)
+    assert orbit_err(two[0][:, keep], one[0][:, keep]) < 1e-13
+    assert spin_err(two[0][:, keep], one[0][:, keep]) < 1e-13
+    assert np.array_equal(two[0][:, ~keep], st[:, ~keep])          # a lost particle's entries are left alone (gst.h)
+    assert np.max(np.abs(two[2] - one[2])) < 1e-13 and two[4] == one[4]
+    ref, rlost, g_ref = O.track(lat, bm, st, turns, split, n_slices, depth)
+    assert np.array_equal(two[1].astype(bool), rlost.astype(bool))
+    assert orbit_err(two[0][:, keep], ref[:, keep]) < 1e-11 and spin_err(two[0][:, keep], ref[:, keep]) < 1e-11
 
 
 def test_failed_rotating_launch_is_reported_by_every_synchronising_call(gst):
