@@ -165,8 +165,11 @@ gst_status gst_track_pwc(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, 
  *                      particles = 3.46 warps each), the turns are cut into chunks and the warps of particles rotate
  *                      over all resident warp slots (csrc/track_chain_kernel.cuh, a cooperative launch)
  *                      Bunches of at most two warps per sub-partition take a kernel variant compiled with registers to
- *                      spare ("track_kernel_fat", see gst_bunch_last_kernel)
- *   GST_LAUNCH_STATIC  never rotate: every warp keeps its slot for the whole call
+ *                      spare ("track_kernel_fat", see gst_bunch_last_kernel), and the smallest ones (at most 4 warps of
+ *                      particles per SM: 18 944 particles on a B200; second-order splits, lattice resident in shared
+ *                      memory) the kernel that gives a particle's orbit and its spin to two warps of a block
+ *                      ("track_split_kernel", csrc/track_split_kernel.cuh)
+ *   GST_LAUNCH_STATIC  never rotate, one thread per particle: every warp keeps its slot for the whole call
  *   GST_LAUNCH_LEAN    as GST_LAUNCH_STATIC, and always the occupancy-oriented kernel, whatever the bunch size        */
 typedef enum { GST_LAUNCH_AUTO = 0, GST_LAUNCH_STATIC = 1, GST_LAUNCH_LEAN = 2 } gst_launch_mode;
 gst_status gst_bunch_set_launch(gst_bunch* b, gst_launch_mode mode);
@@ -189,7 +192,9 @@ gst_status gst_emittance(gst_bunch* b, void* cuda_stream, double out_exy[2]);
  * with registers to spare, taken for bunches of at most two warps per SM sub-partition (37 888 particles on a B200),
  * where one warp's dependency chains set the time -- the same source compiled a second time, so results agree
  * with "track_kernel" to rounding (1e-13), not bit for bit; "track_chain_kernel" IS bit-identical to
- * "track_kernel".                                                                                     */
+ * "track_kernel"; "track_split_kernel": orbit and Omega of 32 particles in one warp, their quaternion work in a
+ * second one (GST_LAUNCH_AUTO, the smallest bunches) -- the same functions compiled once more, so again equal to
+ * the others to rounding.                                                                             */
 const char* gst_bunch_last_kernel(const gst_bunch* b);
 
 /* Copy the lost flags (1 = lost) to HOST memory, n bytes; synchronises the stream and reports a failed

@@ -36,7 +36,8 @@ gst_status gst_diag_chain_poll_limit(gst_bunch* b, int64_t polls);
 /* Registers per thread, stack frame (bytes of local memory per thread) and resident blocks per SM of the tracking
  * kernel of (split, romberg_depth): what bench.py compares with the ncu capture its flop model came from.
  * variant: 0 = track_kernel, 1 = track_chain_kernel (second-order splits), 2 = track_kernel_fat (the small-bunch
- * variant, see gst_bunch_last_kernel).  HOST out pointers, any may be NULL.                               */
+ * variant, see gst_bunch_last_kernel), 3 = track_split_kernel (second-order splits).  HOST out pointers, any may
+ * be NULL.                                                                                                */
 gst_status gst_diag_kernel_info(gst_split split, int romberg_depth, int variant, int* out_registers,
                                 int* out_local_bytes, int* out_max_blocks_per_sm);
 
