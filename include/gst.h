@@ -165,8 +165,8 @@ gst_status gst_track_pwc(gst_bunch* b, const gst_lattice* lat, int64_t n_turns, 
  *                      particles = 3.46 warps each), the turns are cut into chunks and the warps of particles rotate
  *                      over all resident warp slots (csrc/track_chain_kernel.cuh, a cooperative launch)
  *                      Bunches of at most two warps per sub-partition take a kernel variant compiled with registers to
- *                      spare ("track_kernel_fat", see gst_bunch_last_kernel), and the smallest ones (at most 4 warps of
- *                      particles per SM: 18 944 particles on a B200; second-order splits, lattice resident in shared
+ *                      spare ("track_kernel_fat", see gst_bunch_last_kernel), and the smallest ones (at most 3 warps of
+ *                      particles per SM: 14 208 particles on a B200; second-order splits, lattice resident in shared
  *                      memory) the kernel that gives a particle's orbit and its spin to two warps of a block
  *                      ("track_split_kernel", csrc/track_split_kernel.cuh)
  *   GST_LAUNCH_STATIC  never rotate, one thread per particle: every warp keeps its slot for the whole call

@@ -113,7 +113,7 @@ inline bool chain_plan(long long n, long long n_turns, long long steps_per_turn,
 // Bunches that take the two-warp kernel: its 2 x ceil(n / 32) warps each find a sub-partition of their own.
 // GST_SPLIT_MAX_WARPS_PER_SM (a build-time override for measurements) counts particle warps per SM.
 #ifndef GST_SPLIT_MAX_WARPS_PER_SM
-#define GST_SPLIT_MAX_WARPS_PER_SM 4
+#define GST_SPLIT_MAX_WARPS_PER_SM 3
 #endif
 inline long long split_max_warps(int sms) { return (long long)GST_SPLIT_MAX_WARPS_PER_SM * sms; }
 

@@ -34,23 +34,36 @@ enum : int { RING_FULL = 1, RING_EMPTY = 3 };
 __device__ __forceinline__ void named_sync(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
 __device__ __forceinline__ void named_arrive(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
 
-// One lane's view of the ring: entry r, component k of lane l at double [r * 96 + k * 32 + l].
+__device__ __forceinline__ void sts_f64(unsigned addr, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory"); }
+__device__ __forceinline__ double lds_f64(unsigned addr) {
+  double v;
+  asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr) : "memory");
+  return v;
+}
+
+// One lane's view of the ring: entry r, component k of lane l at byte r * 768 + k * 256 + l * 8 of the ring (shared
+// state space, 32-bit addresses).  Half h is entries 16 h .. 16 h + 15.  The producer waits for "half h empty" before
+// it writes the half's first entry and announces "half h full" after its last; the consumer the other way round.
+// Nothing depends on the absolute count, so the 32-bit counter may wrap (it does after 4.3e9 edges, under a million
+// turns of a large ring).
 struct RotvecRing {
-  double* mine;      // ring + lane
+  unsigned mine;     // shared-space address of this lane's slot in entry 0
   unsigned s;        // entries pushed (producer) or popped (consumer) so far; both count the same sequence
+  __device__ __forceinline__ void attach(const void* ring, int lane) {
+    mine = (unsigned)__cvta_generic_to_shared(ring) + 8u * (unsigned)lane;
+    s = 0;
+  }
   // producer -------------------------------------------------------------------------------------------------
   __device__ __forceinline__ void push(double wx, double wy, double ws) {
-    if ((s & (SPLIT_HALF - 1)) == 0) {
-      const int h = (s / SPLIT_HALF) & 1;
-      if (s != 0) named_arrive(RING_FULL + (h ^ 1));     // the half just written may be read
-      named_sync(RING_EMPTY + h);                        // wait until this half has been read
-    }
-    double* p = mine + (s & (2 * SPLIT_HALF - 1)) * 96;
-    p[0] = wx; p[32] = wy; p[64] = ws;
+    const unsigned t = s & (SPLIT_HALF - 1), h = (s / SPLIT_HALF) & 1;
+    if (t == 0) named_sync(RING_EMPTY + h);              // wait until this half has been read
+    const unsigned p = mine + (s & (2 * SPLIT_HALF - 1)) * 768u;
+    sts_f64(p, wx); sts_f64(p + 256, wy); sts_f64(p + 512, ws);
+    if (t == SPLIT_HALF - 1) named_arrive(RING_FULL + h);   // the half just written may be read
     ++s;
   }
-  __device__ __forceinline__ void flush() {              // the last, possibly partial, half
-    if (s != 0) named_arrive(RING_FULL + (((s - 1) / SPLIT_HALF) & 1));
+  __device__ __forceinline__ void flush() {              // the last half, if it is a partial one
+    if ((s & (SPLIT_HALF - 1)) != 0) named_arrive(RING_FULL + ((s / SPLIT_HALF) & 1));
   }
   // consumer -------------------------------------------------------------------------------------------------
   __device__ __forceinline__ void open() {               // both halves start empty
@@ -58,13 +71,11 @@ struct RotvecRing {
     named_arrive(RING_EMPTY + 1);
   }
   __device__ __forceinline__ void pop(double& wx, double& wy, double& ws) {
-    if ((s & (SPLIT_HALF - 1)) == 0) {
-      const int h = (s / SPLIT_HALF) & 1;
-      if (s != 0) named_arrive(RING_EMPTY + (h ^ 1));    // the half just read may be written again
-      named_sync(RING_FULL + h);
-    }
-    const double* p = mine + (s & (2 * SPLIT_HALF - 1)) * 96;
-    wx = p[0]; wy = p[32]; ws = p[64];
+    const unsigned t = s & (SPLIT_HALF - 1), h = (s / SPLIT_HALF) & 1;
+    if (t == 0) named_sync(RING_FULL + h);
+    const unsigned p = mine + (s & (2 * SPLIT_HALF - 1)) * 768u;
+    wx = lds_f64(p); wy = lds_f64(p + 256); ws = lds_f64(p + 512);
+    if (t == SPLIT_HALF - 1) named_arrive(RING_EMPTY + h);  // the half just read may be written again
     ++s;
   }
 };
@@ -167,8 +178,7 @@ __global__ void __launch_bounds__(SPLIT_BLOCK, SPLIT_MIN_BLOCKS) track_split_ker
   const long long j = (long long)blockIdx.x * 32 + lane;
   const bool valid = j < a.n && !a.lost[j];
   RotvecRing ring;
-  ring.mine = reinterpret_cast<double*>(smem_raw + split_ring_offset(a.n_unique, a.n_seq)) + lane;
-  ring.s = 0;
+  ring.attach(smem_raw + split_ring_offset(a.n_unique, a.n_seq), lane);
   State z;
   z.X = z.Px = z.Y = z.Py = z.T = z.Pt = 0.0;
   z.Sx = 0.0; z.Sy = 1.0; z.Ss = 0.0;
