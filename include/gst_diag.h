@@ -27,6 +27,14 @@ gst_status gst_diag_fp64_peak_rrr(double* out_tflops, double* out_ms);
  * max |sqrt(x)*rsqrt(x) - 1|} in units of 2^-53.                                                   */
 gst_status gst_diag_selftest_math(double out[2]);
 
+/* Self-test of the shared-memory ring through which the two-warp kernel (csrc/track_split_kernel.cuh) hands rotation
+ * vectors from its orbit warp to its spin warp: one block, warp 0 pushes `n_entries` entries, warp 1 pops and compares
+ * them; both start their 32-bit entry counter at `start_count` (a multiple of 32, the ring length; GST_EINVAL
+ * otherwise), so that a start just below 2^32 takes the protocol through the wrap of the counter.  HOST out = number
+ * of values that came out wrong (0 expected).  A broken protocol shows as a mismatch count or as a launch that
+ * never ends: call it under a timeout.                                                                          */
+gst_status gst_diag_selftest_ring(uint32_t start_count, uint32_t n_entries, int64_t* out_mismatches);
+
 /* Fault injection for the rotating launch (csrc/track_chain_kernel.cuh): a warp that waits for a hand-off
  * gives up after `polls` polls whatever progress the rest of the chip makes (0 restores the progress-based
  * limit).  With a small value the next rotating gst_track on this bunch fails the way a hung hand-off

@@ -72,6 +72,29 @@ __global__ void math_selftest_kernel(unsigned long long* out, int n) {
   atomicMax(out + 1, (unsigned long long)__double_as_longlong(worst_rsq));
 }
 
+// The rotation-vector ring of track_split_kernel.cuh on its own: warp 0 pushes n entries, warp 1 pops and checks them.
+// Both start their entry counter at `start` (a multiple of the ring length), e.g. just below the wrap of 32 bits.
+__global__ void __launch_bounds__(SPLIT_BLOCK) ring_selftest_kernel(unsigned start, unsigned n, unsigned long long* bad) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int lane = threadIdx.x & 31;
+  RotvecRing ring;
+  ring.attach(smem_raw, lane);
+  ring.s = start;
+  if (threadIdx.x < 32) {
+    for (unsigned i = 0; i < n; ++i) ring.push(1.0 * i + 0.001 * lane, -2.0 * i + lane, 0.5 * i);
+    ring.flush();
+  } else {
+    ring.open();
+    unsigned long long wrong = 0;
+    for (unsigned i = 0; i < n; ++i) {
+      double x, y, z;
+      ring.pop(x, y, z);
+      wrong += (x != 1.0 * i + 0.001 * lane) + (y != -2.0 * i + lane) + (z != 0.5 * i);
+    }
+    if (wrong) atomicAdd(bad, wrong);
+  }
+}
+
 }  // namespace gst
 
 namespace {
@@ -137,6 +160,21 @@ gst_status gst_diag_selftest_math(double out[2]) {
 #ifndef GST_KERNEL_SOURCE_HASH
 #define GST_KERNEL_SOURCE_HASH "unknown"
 #endif
+gst_status gst_diag_selftest_ring(uint32_t start_count, uint32_t n_entries, int64_t* out_mismatches) {
+  if (!out_mismatches) return fail(GST_EINVAL, "null argument");
+  if (start_count % (2 * gst::SPLIT_HALF) != 0) return fail(GST_EINVAL, "start_count must be a multiple of the ring length, %d", 2 * gst::SPLIT_HALF);
+  unsigned long long* d = nullptr;
+  CUDA_TRY(cudaMalloc(&d, 8));
+  CUDA_TRY(cudaMemset(d, 0, 8));
+  gst::ring_selftest_kernel<<<1, gst::SPLIT_BLOCK, gst::SPLIT_RING_BYTES>>>(start_count, n_entries, d);
+  unsigned long long h = 0;
+  cudaError_t ce = cudaMemcpy(&h, d, 8, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (ce != cudaSuccess) return fail(GST_ECUDA, "ring selftest: %s", cudaGetErrorString(ce));
+  *out_mismatches = (int64_t)h;
+  return GST_OK;
+}
+
 const char* gst_diag_kernel_source_hash(void) { return GST_KERNEL_SOURCE_HASH; }
 
 gst_status gst_diag_kernel_info(gst_split split, int romberg_depth, int variant, int* out_registers, int* out_local_bytes,

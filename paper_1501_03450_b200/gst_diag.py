@@ -5,8 +5,8 @@ import ctypes as C
 
 from . import gst
 
-EXPORTS = ["gst_diag_fp64_peak", "gst_diag_fp64_peak_rrr", "gst_diag_selftest_math", "gst_diag_chain_poll_limit",
-           "gst_diag_kernel_info", "gst_diag_kernel_source_hash"]
+EXPORTS = ["gst_diag_fp64_peak", "gst_diag_fp64_peak_rrr", "gst_diag_selftest_math", "gst_diag_selftest_ring",
+           "gst_diag_chain_poll_limit", "gst_diag_kernel_info", "gst_diag_kernel_source_hash"]
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int)
 _ready = False
@@ -19,6 +19,7 @@ def lib():
         L.gst_diag_fp64_peak.argtypes = [_dp, _dp]
         L.gst_diag_fp64_peak_rrr.argtypes = [_dp, _dp]
         L.gst_diag_selftest_math.argtypes = [_dp]
+        L.gst_diag_selftest_ring.argtypes = [C.c_uint32, C.c_uint32, C.POINTER(C.c_int64)]
         L.gst_diag_chain_poll_limit.argtypes = [C.c_void_p, C.c_int64]
         L.gst_diag_kernel_info.argtypes = [C.c_int, C.c_int, C.c_int, _ip, _ip, _ip]
         for name in EXPORTS:
@@ -50,6 +51,13 @@ def selftest_math():
     out = (C.c_double * 2)()
     gst._check(lib().gst_diag_selftest_math(out))
     return out[0], out[1]
+
+
+def selftest_ring(start_count, n_entries):
+    """gst_diag_selftest_ring: values that came out of the two-warp kernel's ring wrong (0 expected)."""
+    bad = C.c_int64(-1)
+    gst._check(lib().gst_diag_selftest_ring(int(start_count), int(n_entries), C.byref(bad)))
+    return bad.value
 
 
 def chain_poll_limit(bunch, polls):

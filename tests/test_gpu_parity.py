@@ -410,6 +410,19 @@ def test_two_warp_kernel_agrees_with_the_fused_kernel(gst, O, split, depth, n_sl
     assert orbit_err(two[0][:, keep], ref[:, keep]) < 1e-11 and spin_err(two[0][:, keep], ref[:, keep]) < 1e-11
 
 
+@pytest.mark.timeout(120)
+@pytest.mark.parametrize("start,n", [(0, 1), (0, 15), (0, 16), (0, 17), (0, 32), (0, 1000), (2**32 - 32, 16), (2**32 - 32, 33),
+                                     (2**32 - 64, 1000), (2**31 - 32, 100)])
+def test_ring_of_the_two_warp_kernel_across_the_wrap_of_its_counter(gst, start, n):
+    """The ring that carries rotation vectors from the orbit warp to the spin warp (csrc/track_split_kernel.cuh) counts
+    its entries in 32 bits: 4.3e9 edges are under a million turns of a large ring in one gst_track.  Its protocol looks
+    at the position within a half only, so the count may wrap; partial and exactly full last halves included."""
+    from paper_1501_03450_b200 import gst_diag
+    assert gst_diag.selftest_ring(start, n) == 0
+    with pytest.raises(Exception):
+        gst_diag.selftest_ring(start + 7, n)
+
+
 def test_failed_rotating_launch_is_reported_by_every_synchronising_call(gst):
     """Fault injection (include/gst_diag.h): with a poll budget of one, the first warp that has to wait for a
     hand-off gives up as it would after a hang.  Every call that synchronises must then return GST_ECUDA once,
