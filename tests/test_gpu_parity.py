@@ -410,6 +410,24 @@ def test_two_warp_kernel_agrees_with_the_fused_kernel(gst, O, split, depth, n_sl
     assert orbit_err(two[0][:, keep], ref[:, keep]) < 1e-11 and spin_err(two[0][:, keep], ref[:, keep]) < 1e-11
 
 
+@pytest.mark.parametrize("n,turns,kernel", [(1, 1, "track_split_kernel"), (14208, 1, "track_split_kernel"), (14209, 1, "track_kernel_fat"),
+                                            (37888, 16, "track_kernel_fat"), (37889, 1, "track_kernel"),
+                                            (37920, 16, "track_chain_kernel"), (65536, 15, "track_kernel"),
+                                            (65536, 16, "track_chain_kernel"), (148 * 8 * 64, 16, "track_kernel")])
+def test_launch_planner_picks_the_kernel_by_bunch_size(gst, n, turns, kernel):
+    """csrc/track_launch.cuh on a B200 (148 SMs): the two-warp kernel up to 3 warps of particles per SM, the small-bunch
+    build of the fused kernel up to 2 warps per sub-partition, the rotating launch where one wave fills the
+    sub-partitions unevenly and there are at least 16 turns, else one thread per particle with its slot for the whole
+    call (a bunch that fills every warp slot exactly included)."""
+    if torch.cuda.get_device_properties(0).multi_processor_count != 148:
+        pytest.skip("the sizes are those of a 148-SM B200")
+    lat = W.lattice([W.drift(1.0), W.quad(0.5, 0.3), W.drift(1.0), W.sbend(2.0, 0.1), W.quad(0.5, -0.3)])
+    bm = W.beam(25.0)
+    st = W.gaussian_bunch(3, n, 25.0, 1e-3, 1e-4, 1e-3, 1e-4, 1e-4, 0.05, "sphere")
+    out, lost, pol, emit, g1 = gpu_track(gst, lat, bm, st, turns, W.SPLIT_BEND_KICK, 2, 2, want_kernel=kernel)
+    assert not lost.any() and np.all(np.isfinite(out))
+
+
 @pytest.mark.timeout(120)
 @pytest.mark.parametrize("start,n", [(0, 1), (0, 15), (0, 16), (0, 17), (0, 32), (0, 1000), (2**32 - 32, 16), (2**32 - 32, 33),
                                      (2**32 - 64, 1000), (2**31 - 32, 100)])
