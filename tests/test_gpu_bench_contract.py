@@ -5,6 +5,7 @@ under torchrun with one rank (the N > 1 launch: NCCL rendezvous on 127.0.0.1, ba
 and the reference arm (the oracle on the host cores)."""
 import json
 import os
+import socket
 import subprocess
 import sys
 
@@ -53,8 +54,11 @@ def test_bench_line_of_the_default_launch():
 
 
 def test_bench_line_under_torchrun_with_one_rank():
+    with socket.socket() as sk:                          # a port that is free right now
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
     d = run_bench([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "1", "--master-addr",
-                   "127.0.0.1", "--master-port", "29731", "bench.py", "--gpus", "1"] + SHORT + ["--no-cpu-baseline"])
+                   "127.0.0.1", "--master-port", str(port), "bench.py", "--gpus", "1"] + SHORT + ["--no-cpu-baseline"])
     check_line(d, 1)
     assert "particle shards x1" in d["config"]["parallelism"]
 
