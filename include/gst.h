@@ -187,6 +187,23 @@ gst_status gst_polarization(gst_bunch* b, void* cuda_stream, double out[4], int6
 /* Geometric rms emittances (a13; reading A19), HOST out = {eps_x, eps_y}; synchronises the stream. */
 gst_status gst_emittance(gst_bunch* b, void* cuda_stream, double out_exy[2]);
 
+/* The ADDITIVE record behind both reports, for bunches sharded over several GPUs (particles are
+ * independent, so the only exchange of the method is the sum behind a bunch-wide report).  HOST out:
+ *   [0..3]   sum Sx, sum Sy, sum Ss, number of particles not lost                                     (A18)
+ *   [4..7]   sum X, sum Px, sum Y, sum Py
+ *   [8..13]  central sums about THIS shard's means: dX dX, dPx dPx, dX dPx, dY dY, dPy dPy, dY dPy    (A19, two-pass)
+ *   [14..19] n m m' of the same six pairs (m = this shard's means)
+ * Records of disjoint shards add component by component (one all-reduce of GST_MOMENTS_LEN doubles); the central sums
+ * of the union are [8..13] + [14..19] - (sum u)(sum u')/n of the summed record, which gst_moments_finish evaluates.
+ * Synchronises the stream and reports a failed launch like gst_polarization.                                        */
+#define GST_MOMENTS_LEN 20
+gst_status gst_moments(gst_bunch* b, void* cuda_stream, double out[GST_MOMENTS_LEN]);
+
+/* Polarization {Px, Py, Ps, |P|} (A18), geometric rms emittances {eps_x, eps_y} (A19) and particle count of a record
+ * of gst_moments or of a component-wise sum of such records.  HOST pointers; any of the three outputs may be NULL.
+ * Pure host arithmetic: needs no device.  For a single record it returns what gst_polarization / gst_emittance do.  */
+gst_status gst_moments_finish(const double rec[GST_MOMENTS_LEN], double out_pol[4], double out_exy[2], int64_t* out_alive);
+
 /* Name of the kernel the last gst_track / gst_track_pwc on this bunch launched ("" before the first call; static
  * storage): "track_kernel"; "track_chain_kernel" (the rotating launch); "track_kernel_fat": the same code compiled
  * with registers to spare, taken for bunches of at most two warps per SM sub-partition (37 888 particles on a B200),

@@ -610,6 +610,55 @@ gst_status gst_emittance(gst_bunch* b, void* cuda_stream, double out_exy[2]) {
   return GST_OK;
 }
 
+// 8(e): the additive record of a shard.  Central sums about the shard's own means (two-pass, moments_kernel<true>)
+// plus n * mean * mean per pair, so that the records of disjoint shards add component by component and
+//   central sum of the union = sum c + sum n m m' - (sum u)(sum u')/alive      (gst_moments_finish).
+gst_status gst_moments(gst_bunch* b, void* cuda_stream, double out[GST_MOMENTS_LEN]) {
+  if (!b || !out) return fail(GST_EINVAL, "null argument");
+  GUARD_DEVICE(b->device);
+  gst_status s = run_moments(b, (cudaStream_t)cuda_stream, true);
+  if (s != GST_OK) return s;
+  const double* r = b->h_result;                    // {sum Sx, Sy, Ss, alive, sum X, Px, Y, Py}
+  const double* c = b->h_result + gst::RED_WIDTH;   // {sxx, spp, sxp, syy, sqq, syq} about this shard's means
+  for (int k = 0; k < 8; ++k) out[k] = r[k];
+  const double alive = r[3];
+  const double inv = alive > 0 ? 1.0 / alive : 0.0;
+  for (int k = 0; k < 2; ++k) {
+    const double su = r[4 + 2 * k], sp = r[5 + 2 * k];
+    out[8 + 3 * k] = alive > 0 ? c[3 * k] : 0.0;
+    out[9 + 3 * k] = alive > 0 ? c[3 * k + 1] : 0.0;
+    out[10 + 3 * k] = alive > 0 ? c[3 * k + 2] : 0.0;
+    out[14 + 3 * k] = su * su * inv;
+    out[15 + 3 * k] = sp * sp * inv;
+    out[16 + 3 * k] = su * sp * inv;
+  }
+  return GST_OK;
+}
+
+gst_status gst_moments_finish(const double rec[GST_MOMENTS_LEN], double out_pol[4], double out_exy[2], int64_t* out_alive) {
+  if (!rec) return fail(GST_EINVAL, "null argument");
+  const double alive = rec[3];
+  if (!(alive >= 0) || alive != std::floor(alive)) return fail(GST_EINVAL, "record with a particle count of %g", alive);
+  const double inv = alive > 0 ? 1.0 / alive : 0.0;
+  if (out_alive) *out_alive = (int64_t)alive;
+  if (out_pol) {
+    out_pol[0] = rec[0] * inv; out_pol[1] = rec[1] * inv; out_pol[2] = rec[2] * inv;
+    out_pol[3] = std::sqrt(out_pol[0] * out_pol[0] + out_pol[1] * out_pol[1] + out_pol[2] * out_pol[2]);
+  }
+  if (out_exy) {
+    for (int k = 0; k < 2; ++k) {
+      const double su = rec[4 + 2 * k], sp = rec[5 + 2 * k];
+      // between-shard part of the central sums: sum_r n_r m_r m_r' - n m m'  (zero for a single shard)
+      const double uu = (rec[8 + 3 * k] + (rec[14 + 3 * k] - su * su * inv)) * inv;
+      const double pp = (rec[9 + 3 * k] + (rec[15 + 3 * k] - sp * sp * inv)) * inv;
+      const double up = (rec[10 + 3 * k] + (rec[16 + 3 * k] - su * sp * inv)) * inv;
+      const double e2 = uu * pp - up * up;
+      out_exy[k] = e2 > 0 ? std::sqrt(e2) : 0.0;
+    }
+  }
+  return GST_OK;
+}
+
 gst_status gst_bunch_lost(gst_bunch* b, void* cuda_stream, uint8_t* host_out) {
   if (!b || !host_out) return fail(GST_EINVAL, "null argument");
   GUARD_DEVICE(b->device);

@@ -40,8 +40,9 @@ EXPORTS = ["gst_lattice_create", "gst_lattice_destroy", "gst_lattice_steps_per_t
            "gst_bunch_destroy", "gst_track", "gst_polarization", "gst_emittance", "gst_bunch_lost",
            "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host", "gst_last_error",
            "gst_bunch_set_launch", "gst_bunch_status", "gst_track_pwc", "gst_bunch_last_kernel",
-           "gst_polarization_noalloc"]
+           "gst_polarization_noalloc", "gst_moments", "gst_moments_finish"]
 NOALLOC_MAX_PARTICLES = 1 << 20
+MOMENTS_LEN = 20
 LAUNCH_AUTO, LAUNCH_STATIC, LAUNCH_LEAN = 0, 1, 2
 
 
@@ -70,6 +71,8 @@ def lib():
         L.gst_bunch_last_kernel.restype = C.c_char_p
         L.gst_polarization.argtypes = [vp, vp, _dp, C.POINTER(C.c_int64)]
         L.gst_emittance.argtypes = [vp, vp, _dp]
+        L.gst_moments.argtypes = [vp, vp, _dp]
+        L.gst_moments_finish.argtypes = [_dp, _dp, _dp, C.POINTER(C.c_int64)]
         L.gst_bunch_lost.argtypes = [vp, vp, C.POINTER(C.c_uint8)]
         L.gst_bunch_reference.argtypes = [vp, _dp, C.POINTER(C.c_int64)]
         L.gst_bunch_set_reference.argtypes = [vp, C.POINTER(gst_beam), C.c_int64]
@@ -81,7 +84,7 @@ def lib():
         L.gst_bunch_status.argtypes = [vp, vp]
         for name in ("gst_lattice_create", "gst_bunch_init", "gst_track", "gst_polarization", "gst_emittance",
                      "gst_bunch_lost", "gst_bunch_reference", "gst_bunch_set_reference", "gst_track_host",
-                     "gst_bunch_set_launch", "gst_bunch_status"):
+                     "gst_bunch_set_launch", "gst_bunch_status", "gst_moments", "gst_moments_finish"):
             getattr(L, name).restype = C.c_int
         _lib = L
     return _lib
@@ -209,6 +212,12 @@ class Bunch:
         _check(lib().gst_emittance(self._h, self._stream(stream), out))
         return np.array(out[:])
 
+    def moments(self, stream=None):
+        """The shard's additive record (gst_moments): sum it over the shards, then moments_finish()."""
+        out = (C.c_double * MOMENTS_LEN)()
+        _check(lib().gst_moments(self._h, self._stream(stream), out))
+        return np.array(out[:])
+
     def lost(self, stream=None):
         out = np.zeros(max(self.n, 1), dtype=np.uint8)
         _check(lib().gst_bunch_lost(self._h, self._stream(stream), out.ctypes.data_as(C.POINTER(C.c_uint8))))
@@ -234,6 +243,16 @@ class Bunch:
             self.close()
         except Exception:
             pass
+
+
+def moments_finish(record):
+    """gst_moments_finish: (polarization {Px, Py, Ps, |P|}, emittances {eps_x, eps_y}, particles counted) of a record
+    of Bunch.moments() or of a component-wise sum of such records.  Host arithmetic in the library; needs no GPU."""
+    rec = np.ascontiguousarray(record, dtype=np.float64)
+    assert rec.shape == (MOMENTS_LEN,)
+    pol, exy, alive = (C.c_double * 4)(), (C.c_double * 2)(), C.c_int64(0)
+    _check(lib().gst_moments_finish(rec.ctypes.data_as(_dp), pol, exy, C.byref(alive)))
+    return np.array(pol[:]), np.array(exy[:]), alive.value
 
 
 def polarization_noalloc(sx, sy, ss, lost, out, stream=None):

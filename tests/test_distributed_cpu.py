@@ -3,6 +3,7 @@ import os
 import socket
 
 import numpy as np
+import pytest
 import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
@@ -51,6 +52,90 @@ def test_sharded_polarization_equals_whole_bunch():
     ref = S[:, mask].mean(axis=1)
     assert alive == int(mask.sum())
     assert np.max(np.abs(g[:3] - ref)) < 1e-15 and abs(g[3] - np.linalg.norm(ref)) < 1e-15
+
+
+def _record(X, Px, Y, Py, S, alive):
+    """The record of include/gst.h gst_moments, from its definition (numpy)."""
+    S, X, Px, Y, Py = S[:, alive], X[alive], Px[alive], Y[alive], Py[alive]
+    n = float(alive.sum())
+    rec = np.zeros(20)
+    rec[0:3] = S.sum(axis=1)
+    rec[3] = n
+    rec[4:8] = [X.sum(), Px.sum(), Y.sum(), Py.sum()]
+    if n > 0:
+        for k, (u, p) in enumerate(((X, Px), (Y, Py))):
+            du, dp = u - u.mean(), p - p.mean()
+            rec[8 + 3 * k: 11 + 3 * k] = [(du * du).sum(), (dp * dp).sum(), (du * dp).sum()]
+            rec[14 + 3 * k: 17 + 3 * k] = [n * u.mean() ** 2, n * p.mean() ** 2, n * u.mean() * p.mean()]
+    return rec
+
+
+def _bunch(n, seed):
+    rng = np.random.default_rng(seed)
+    X, Px, Y, Py = (rng.normal(size=n) * s for s in (1e-3, 1e-4, 2e-3, 3e-4))
+    Px += 0.3 * X                                                  # correlated planes: the cross term counts
+    X += 5e-3                                                      # offset beam
+    S = rng.normal(size=(3, n))
+    S /= np.linalg.norm(S, axis=0)
+    return X, Px, Y, Py, S, rng.uniform(size=n) > 0.05
+
+
+def _emittance(u, p):
+    return np.sqrt(np.var(u) * np.var(p) - np.mean((u - u.mean()) * (p - p.mean())) ** 2)
+
+
+def test_records_of_shards_add_up_to_the_whole_bunch():
+    """gst_moments_finish (host arithmetic of the library) on a sum of shard records against numpy on the whole
+    bunch: uneven shards, an empty one, one shifted against the others."""
+    from paper_1501_03450_b200 import gst
+    X, Px, Y, Py, S, alive = _bunch(5000, 1)
+    Y[3000:] += 4e-3
+    total = np.zeros(20)
+    for lo, hi in ((0, 1), (1, 1), (1, 3000), (3000, 5000)):
+        total += _record(X[lo:hi], Px[lo:hi], Y[lo:hi], Py[lo:hi], S[:, lo:hi], alive[lo:hi])
+    pol, exy, n_alive = gst.moments_finish(total)
+    assert n_alive == int(alive.sum())
+    assert np.max(np.abs(pol[:3] - S[:, alive].mean(axis=1))) < 1e-15
+    ref = np.array([_emittance(X[alive], Px[alive]), _emittance(Y[alive], Py[alive])])
+    assert np.max(np.abs(exy / ref - 1)) < 1e-12
+    pol1, exy1, _ = gst.moments_finish(_record(X, Px, Y, Py, S, alive))     # one record: the between-shard term is zero
+    assert np.max(np.abs(exy1 / ref - 1)) < 1e-12 and np.max(np.abs(pol1 - pol)) < 1e-15
+    pol0, exy0, n0 = gst.moments_finish(np.zeros(20))                       # nobody left
+    assert n0 == 0 and not pol0.any() and not exy0.any()
+    with pytest.raises(gst.GstError):
+        gst.moments_finish(np.full(20, np.nan))
+
+
+def _report_worker(rank, world, port, out):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    X, Px, Y, Py, S, alive = _bunch(4001, 2)
+    lo, hi = D.shard_bounds(4001, rank, world)
+    rep = D.global_report(_record(X[lo:hi], Px[lo:hi], Y[lo:hi], Py[lo:hi], S[:, lo:hi], alive[lo:hi]))
+    out.put((rank, rep))
+    dist.destroy_process_group()
+
+
+def test_global_report_is_one_allreduce_of_the_records():
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_report_worker, args=(r, 2, port, out)) for r in range(2)]
+    for p in procs:
+        p.start()
+    reps = dict(out.get(timeout=120) for _ in range(2))
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    X, Px, Y, Py, S, alive = _bunch(4001, 2)
+    ref = np.array([_emittance(X[alive], Px[alive]), _emittance(Y[alive], Py[alive])])
+    for rank in (0, 1):                                                      # every rank holds the whole-bunch report
+        pol, exy, n_alive = reps[rank]
+        assert n_alive == int(alive.sum())
+        assert np.max(np.abs(pol[:3] - S[:, alive].mean(axis=1))) < 1e-15
+        assert np.max(np.abs(exy / ref - 1)) < 1e-12
+    assert np.array_equal(reps[0][1], reps[1][1])
 
 
 def test_shard_bounds_cover_everything_once():

@@ -686,6 +686,38 @@ def test_reductions_match_oracle_on_a_large_bunch(gst, O):
     b.close()
 
 
+def test_shard_records_add_up_to_the_whole_bunch(gst, O):
+    """the records of gst_moments of disjoint shards add; gst_moments_finish of the sum is the report of
+    the whole bunch (the all-reduce of distributed.global_report on one device: three uneven shards, offset beam, one
+    shard displaced against the others so that the between-shard term matters)."""
+    rng = np.random.default_rng(13)
+    n = 100_003
+    st = rng.normal(size=(9, n)) * np.array([1e-3, 1e-4, 2e-3, 3e-4, 0.1, 1e-3, 1, 1, 1])[:, None]
+    st[0] += 5e-3
+    cuts = [0, 17, 40_000, n]
+    st[2, cuts[2]:] += 1e-3
+    st[3, cuts[2]:] -= 2e-4
+    total = np.zeros(gst.MOMENTS_LEN)
+    for lo, hi in zip(cuts[:-1], cuts[1:]):
+        d = torch.tensor(st[:, lo:hi], dtype=torch.float64, device="cuda").contiguous()
+        b = gst.Bunch(d)
+        rec = b.moments()
+        pol1, emit1, alive1 = gst.moments_finish(rec)              # a single record = the bunch's own reports
+        pol, _ = b.polarization()
+        assert alive1 == hi - lo and np.array_equal(pol1, pol)
+        assert np.max(np.abs(emit1 / b.emittance() - 1)) < 1e-13
+        total += rec
+        b.close()
+    pol, emit, alive = gst.moments_finish(total)
+    rp, _ = O.polarization(st)
+    assert alive == n and np.max(np.abs(pol - rp)) < 1e-14
+    assert np.max(np.abs(emit / O.emittance(st) - 1)) < 1e-12, emit / O.emittance(st) - 1
+    d = torch.tensor(st, dtype=torch.float64, device="cuda").contiguous()
+    b = gst.Bunch(d)
+    assert np.max(np.abs(emit / b.emittance() - 1)) < 1e-12
+    b.close()
+
+
 # ---------------------------------------------------------------------------------------------
 # RHIC-like ring (configs 3, 4, 5): reduced sizes in full, full size on sampled particles
 # ---------------------------------------------------------------------------------------------
