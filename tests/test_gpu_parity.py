@@ -326,6 +326,33 @@ def test_lost_particles_are_flagged_identically_and_excluded_from_reductions(gst
     assert np.max(np.abs(emit / O.emittance(ref, rlost) - 1)) < 1e-11
 
 
+def test_shard_records_leave_lost_particles_out(gst, O):
+    """gst_moments after tracking, two shards with one lost particle each: the summed record reports the bunch without
+    them (A15, A18, A19), as the oracle's reductions over the whole tracked bunch do."""
+    c = W.config(1)
+    st = c["state"].copy()
+    st[1, 5] = 1.5
+    st[3, 40] = -2.0
+    ref, rlost, _ = O.track(c["lattice"], c["beam"], st, 2, c["split"], 4, 3)
+    assert rlost[5] and rlost[40] and rlost.sum() == 2
+    L = gst.Lattice(c["lattice"], c["beam"])
+    total = np.zeros(gst.MOMENTS_LEN)
+    for lo, hi in ((0, 23), (23, st.shape[1])):
+        d = torch.tensor(st[:, lo:hi], dtype=torch.float64, device="cuda").contiguous()
+        b = gst.Bunch(d)
+        b.track(L, 2, c["split"], 4, 3)
+        rec = b.moments()
+        assert rec[3] == hi - lo - 1
+        total += rec
+        b.close()
+    L.close()
+    pol, emit, alive = gst.moments_finish(total)
+    rp, nl = O.polarization(ref, rlost)
+    assert alive == st.shape[1] - 2 and nl == 2
+    assert np.max(np.abs(pol - rp)) < 1e-13
+    assert np.max(np.abs(emit / O.emittance(ref, rlost) - 1)) < 1e-11
+
+
 def test_chain_rotation_is_bit_identical_to_the_static_launch(gst):
     """65 553 particles fill the sub-partitions unevenly, so the default launch rotates the warps of particles
     over the warp slots in chunks of turns (csrc/track_chain_kernel.cuh); state, lost flags and the ramping
