@@ -167,7 +167,10 @@ def test_config4_ramp_with_a_polarization_report_every_100_turns(gst, O):
            worst_dP_any_report=worst_dp, worst_dgamma_rel=worst_g, P_final=pol[3])
 
 
-SPLITS = [W.SPLIT_DRIFT_KICK, W.SPLIT_BEND_KICK, W.SPLIT_MATRIX_KICK]
+# the three splits of BASELINE configs[4] and their fourth-order compositions (f1), which the committed sweep
+# (profiles/r02_study_sweep_order4.md) runs next to them: 6 x 27 = its 162 points
+SPLITS = [W.SPLIT_DRIFT_KICK, W.SPLIT_BEND_KICK, W.SPLIT_MATRIX_KICK,
+          W.SPLIT_DRIFT_KICK_4, W.SPLIT_BEND_KICK_4, W.SPLIT_MATRIX_KICK_4]
 
 
 @pytest.mark.parametrize("split", SPLITS)
