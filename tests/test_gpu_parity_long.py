@@ -8,11 +8,14 @@
   config 4   256 particles x the full 5000 turns of the ramp (100 keV/turn from G gamma = 45.0 through the intrinsic
              resonance at 12 + Q_y = 45.43) in chunks of 100 turns, bunch polarization compared AT EVERY REPORT (BASELINE
              configs[3]: "report the bunch polarization every 100 turns"), gamma_o(n) against its closed form
-  config 5   all 27 (slices, depth) pairs x 3 splits on 64 particles x 10 turns, three of them at the full 100 turns,
-             and the reference run the sweep measures against (fourth-order matrix-kick, 128 slices, depth 6)
+  config 5   all 27 (slices, depth) pairs x 6 splits (second and fourth order) on 64 particles x 10 turns, three of
+             them at the full 100 turns, and the reference run the sweep measures against (fourth-order matrix-kick,
+             128 slices, depth 6)
+  configs 2, 4, 5 at their FULL bunch sizes (4096, 2^20, 262 144 particles), 100 turns in one launch: config 2 against
+             the oracle on every particle, configs 4 and 5 on 256 sampled particles
 
 Tolerances: north_star's 1e-9 per particle after 100 turns (grown linearly with the turn count beyond that) and 1e-6 on
-the bunch polarization; metrics in tests/parity_metrics.py.  Oracle time on 16 host threads: about three minutes in all.
+the bunch polarization; metrics in tests/parity_metrics.py.  Oracle time on 16 host threads: about four minutes in all.
 With GST_PARITY_REPORT=<file> the measured errors are appended to that file as JSON lines (profiles/rNN_parity_long.md).
 """
 import json
@@ -129,6 +132,44 @@ def test_config3_full_launch_256_sampled_particles(gst, O):
     assert np.max(np.abs(np.linalg.norm(got[6:9], axis=0) - 1)) < 1e-11
     assert abs(pol[3] - np.linalg.norm(got[6:9].mean(axis=1))) < 1e-12
     record("config3 full launch, 256 sampled", orbit_1000=orbit_err_per_particle(sub, ref), spin_1000=spin_err(sub, ref),
+           dP_sample=np.max(np.abs(sub[6:9].mean(axis=1) - rp[:3])), P=pol[3])
+
+
+@pytest.mark.parametrize("cfg,kernel,sampled", [(2, "track_split_kernel", 4096), (4, "track_kernel", 256),
+                                                (5, "track_kernel", 256)])
+def test_full_size_launches_of_configs_2_4_5_first_hundred_turns(gst, O, cfg, kernel, sampled):
+    """The other configurations at their FULL bunch sizes (4096, 2^20 and 262 144 particles), 100 turns in one launch:
+    config 2 against the oracle on every particle (north_star: 1e-9 per particle after 100 turns), configs 4 and 5 --
+    several waves of blocks of the plain kernel -- on 256 sampled particles, first and last included."""
+    c = W.config(cfg)
+    n = c["state"].shape[1]
+    assert n == {2: 4096, 4: 1 << 20, 5: 262144}[cfg]
+    args = (c["split"], c["n_slices"], c["depth"])
+    g = GpuBunch(gst, c["lattice"], c["beam"], c["state"])
+    g.track(100, *args)
+    got = g.read()
+    assert g.b.last_kernel() == kernel, g.b.last_kernel()
+    pol, nlost = g.b.polarization()
+    g_gpu, turn = g.b.reference()
+    g.close()
+    assert nlost == 0 and turn == 100
+    if sampled == n:
+        idx = np.arange(n)
+    else:                                                       # a stride coprime to 32: every lane of a warp occurs
+        idx = (np.arange(sampled) * (n // sampled + 1)) % n
+        idx[0], idx[-1] = 0, n - 1
+        assert np.unique(idx).size == sampled and np.unique(idx % 32).size == 32
+    ref, rlost, g_ref = O.track(c["lattice"], c["beam"], c["state"][:, idx], 100, *args)
+    assert not rlost.any()
+    assert abs(g_gpu - g_ref) <= 3e-15 * g_ref
+    sub = got[:, idx]
+    eo, es = orbit_err_per_particle(sub, ref), spin_err(sub, ref)
+    assert eo < 1e-9 and es < 1e-9, (eo, es)
+    rp, _ = O.polarization(ref)
+    assert np.max(np.abs(sub[6:9].mean(axis=1) - rp[:3])) < 1e-6
+    assert np.max(np.abs(np.linalg.norm(got[6:9], axis=0) - 1)) < 1e-11
+    assert abs(pol[3] - np.linalg.norm(got[6:9].mean(axis=1))) < 1e-12
+    record("config%d full size (%d particles), 100 turns, %d compared" % (cfg, n, sampled), orbit_100=eo, spin_100=es,
            dP_sample=np.max(np.abs(sub[6:9].mean(axis=1) - rp[:3])), P=pol[3])
 
 
